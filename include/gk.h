@@ -1,0 +1,123 @@
+/* gk.h -- C ABI of libgk, the B200 (sm_100a) hot path of the local flux-tube delta-f
+ * gyrokinetic solver of arxiv/paper_2604_06085 ("gyaradax"): one Runge-Kutta stage =
+ * quasineutrality field solve -> linear terms I,II,IV,V,VII,VIII + dissipation -> dealiased
+ * ExB bracket (term III) -> fused RK4 stage update.  Citations are PAPER.md line numbers; R<n>
+ * are the readings listed in DESIGN.md.
+ *
+ * Conventions
+ *   - All data pointers are DEVICE pointers unless the name ends in _host.
+ *   - f:   [species a][vpar j][mu l][s i][kx p+K][ky m], ky fastest, K=(nkx-1)/2, kx index monotone
+ *          from -K to K, ky index m = 0..nky-1 (half spectrum, ky_m = m*ky0).
+ *          storage 0: complex64 (float re, float im); 1: complex fp16 (__half2); 2: complex bf16.
+ *   - phi: [s i][kx p+K][ky m] complex64, always.
+ *   - Caller owns f, phi, rhs and the workspace; the context owns only its coefficient tables.
+ *   - Hot calls (field_solve, rhs, rk4_step, rk4_steps) are asynchronous on the stream given to
+ *     gk_create, never synchronise and never allocate.  gk_fluxes synchronises the stream.
+ *   - Every function returns 0 (GK_OK) or a negative error code; no exception crosses the ABI.
+ *     After GK_ECUDA the context is poisoned (sticky CUDA error); text in gk_last_error().
+ *   - There is no CPU fallback: without a CUDA device gk_create returns GK_ECUDA.
+ */
+#ifndef GK_H
+#define GK_H
+#include <stddef.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum { GK_OK = 0, GK_EINVAL = -1, GK_ENOMEM = -2, GK_ECUDA = -3, GK_EUNSUPPORTED = -4 };
+
+typedef struct gk_ctx gk_ctx; /* opaque */
+
+/* Phase-space grid (R1, R3, R5). */
+typedef struct {
+  int nkx, nky, ns, nvpar, nmu; /* nkx odd, ns >= 4, nvpar >= 4, nky >= 1, nmu >= 1               */
+  double ky0;                   /* ky_m = m*ky0 in k_theta*rho_ref units                          */
+  int ikxspace;                 /* dkx = 2*pi*shat*ky0/ikxspace  */
+  double vpar_max;              /* vpar_j = -vpar_max + (j+1/2)*2*vpar_max/nvpar                   */
+  int mu_grid;                  /* 0 = Gauss-Laguerre in 2*mu, 1 = uniform in v_perp*/
+  double vperp_max;             /* upper end of the uniform v_perp grid                           */
+} gk_grid;
+
+/* One kinetic species: charge number, mass, temperature, density (all relative
+ * to the reference species) and the gradient drives R/L_T, R/L_n. */
+typedef struct { double Z, mass, temp, dens, rlt, rln; } gk_species;
+
+/* s-alpha geometry (formulas: reading R2). */
+typedef struct { double q, shat, eps; } gk_salpha;
+
+/* term_mask bits: debugging/test hook that switches individual terms of the RHS. */
+enum {
+  GK_T_I = 1, GK_T_II = 2, GK_T_IV = 4, GK_T_V = 8, GK_T_VII = 16, GK_T_VIII = 32,
+  GK_T_DISS_S = 64, GK_T_DISS_V = 128, GK_T_HYP = 256, GK_T_III = 512, GK_T_ALL = 1023
+};
+
+typedef struct {
+  int nspecies;            /* number of kinetic species (entries of the gk_species array)         */
+  int adiabatic_electrons; /* 1: adiabatic electrons + zonal flux-surface-average correction (R10)*/
+                           /* 0: all species kinetic, no correction (R11)           */
+  double te, ne;           /* adiabatic-electron temperature and density                          */
+  int nonlinear;           /* 1: include term III                                                 */
+  double disp_par, disp_vp, disp_x, disp_y; /* nu_s, nu_v, nu_x, nu_y (R9)            */
+  int s_closure;           /* 0: upwinded 2nd-order boundary classes; 1: zero ghosts (R7)         */
+  int storage;             /* 0 complex64, 1 complex fp16, 2 complex bf16 (BASELINE config 5; R19)*/
+  int term_mask;           /* <= 0: all terms                                                     */
+  int pad_mx, pad_my;      /* padded real-space grid of the bracket; 0 = automatic (R14).  Must be
+                              >= 3K+1 / 3(nky-1)+1 and of the form 2^a * 3^b, b <= 1, <= 256      */
+} gk_opts;
+
+/* Builds all create-time tables (grids, weights, geometry, F_M, J0, Gamma0, Poisson denominators,
+ * connectivity classes, stencil table: PAPER.md:65, 336) on the host in double precision, uploads
+ * them, and binds the context to `cuda_stream` (a cudaStream_t cast to void*, NULL = default
+ * stream).  Errors: GK_EINVAL (bad sizes/null pointers), GK_EUNSUPPORTED (padded grid does not fit
+ * the shared-memory strategy), GK_ENOMEM, GK_ECUDA. */
+int gk_create(const gk_grid *grid, const gk_species *species, const gk_salpha *geom,
+              const gk_opts *opts, void *cuda_stream, gk_ctx **out);
+int gk_destroy(gk_ctx *ctx);
+
+/* Bytes of caller-owned device scratch the hot calls need: moment partial sums, two stage states,
+ * the RK accumulator, spill space of the bracket kernel.  gk_field_solve and gk_rhs need only the
+ * first gk_workspace_bytes_rhs() bytes of it. */
+size_t gk_workspace_bytes(const gk_ctx *ctx);
+size_t gk_workspace_bytes_rhs(const gk_ctx *ctx);
+/* `dev` must be 256-byte aligned and stay valid until replaced or the context is destroyed.
+ * GK_EINVAL if too small for gk_workspace_bytes_rhs(); rk4 calls check for the full size. */
+int gk_set_workspace(gk_ctx *ctx, void *dev, size_t bytes);
+
+/* Quasineutrality field solve: phi(i,p,m) from f.  phi(kx=0,ky=0) = 0. */
+int gk_field_solve(gk_ctx *ctx, const void *f_dev, void *phi_dev);
+
+/* Full right-hand side: solves phi (written to phi_dev), then
+ * rhs = I + II + IV + V + VII + VIII + dissipation + III.  rhs_dev has the layout and storage type
+ * of f and must not alias it. */
+int gk_rhs(gk_ctx *ctx, const void *f_dev, void *phi_dev, void *rhs_dev);
+
+/* One classical RK4 step, phi re-solved at each of the 4 stages; f in-out.
+ * gk_rk4_steps does `nsteps` steps (the paper's gksolve/scan) and keeps the
+ * velocity-space moments of f_{n+1} from the last stage's epilogue for the next step. */
+int gk_rk4_step(gk_ctx *ctx, void *f_dev, double dt);
+int gk_rk4_steps(gk_ctx *ctx, void *f_dev, double dt, int nsteps);
+
+/* Transport fluxes per species (R18): out_host[3*a + {0,1,2}] = particle, heat,
+ * parallel-momentum flux.  Synchronises the stream. */
+int gk_fluxes(gk_ctx *ctx, const void *f_dev, const void *phi_dev, double *out_host);
+
+/* Test hook: copies a create-time table to host memory as doubles.  `which` is one of
+ * "vpar","mu","wmu","kx","ky","B","F","BG","J0","Gamma0","FM","den","zonal","pad".  Returns the
+ * number of doubles (also when host_out is NULL), 0 for an unknown name. */
+size_t gk_export_table(const gk_ctx *ctx, const char *which, double *host_out, size_t max_doubles);
+
+/* Number of kernel launches issued through this context so far (bench.py's gpu_launches). */
+long long gk_launch_count(const gk_ctx *ctx);
+/* CUDA-event time (ms) spent in the stage kernel since the last call with reset!=0, and the number
+ * of stage-kernel launches in that interval; events are recorded on the context stream only while
+ * profiling is enabled with gk_set_profiling(ctx, 1).  Synchronises the stream. */
+int gk_set_profiling(gk_ctx *ctx, int on);
+int gk_stage_kernel_time(gk_ctx *ctx, double *ms_total, long long *launches, int reset);
+
+const char *gk_last_error(const gk_ctx *ctx); /* never NULL; "" if no error */
+const char *gk_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif
