@@ -1,0 +1,62 @@
+// gk_dev.h -- device-side parameter block of libgk (product path; shares nothing with oracle/).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#define GK_MAX_SPECIES 4
+
+// Per-species scalars, float copies of the host doubles.
+struct GkSpeciesDev {
+  float Z, T, mass, dens, vR, rlt, rln;
+  float ToverZ, ZoverT;
+  float momfac;  // Z n 2 pi w_v : species factor of the velocity-space moment (B_i, w_mu applied per point)
+};
+
+// Everything the kernels need that is not f itself.  Passed by value (__grid_constant__).
+struct GkDev {
+  int nsp, nv, nmu, ns, nkx, nky, K, ikx;
+  int mx, my;        // padded real-space grid of the bracket (R14)
+  int ldx;           // row stride (float2) of the x-transformed half-spectrum arrays  [mx][ldx]
+  int ldy;           // row stride (float2) of real-space rows                          [rows][ldy]
+  int rc;            // rows per chunk of the y-transform workspace (even, divides mx)
+  int adiabatic, mask, storage;
+  int jchunk, nchunk;  // vpar chunking of the stage kernel's work items
+  int nparts;          // number of moment partial planes = nsp*nmu*nchunk
+  int gchi_in_smem;    // 1: real-space grad(chi) lives in shared memory, 0: per-CTA global scratch
+  float ds_inv, dv_inv;
+  float nu_s, nu_v;
+  float ae;            // ne/Te of the adiabatic electrons
+  float fftnorm;       // 1/(mx*my)
+  long long slab;      // nkx*nky
+  long long nphi;      // ns*nkx*nky
+  long long ntot;
+  // tables (device pointers, float)
+  const float *v, *fmv;             // [nv]  vpar_j, pi^-3/2 exp(-v^2)
+  const float *mu, *wmu;            // [nmu]
+  const float *fmm;                 // [nmu][ns] exp(-2 mu B)
+  const float *B, *F, *BG, *sth, *cz, *Rmaj;  // [ns]
+  const float *kx, *ky;             // [nkx], [nky]
+  const float *hypx, *hypy;         // nu_x (kx/kxmax)^4, nu_y (ky/kymax)^4
+  const float *J0;                  // [nsp][nmu][ns][nkx][nky]
+  const float *dinv;                // [ns][nkx][nky] 1/(A+ae) or 1/A; 0 at (kx,ky)=(0,0)
+  const float *zinv;                // [nkx] 1/<A/(A+ae)>_s, 0 at kx=0 (adiabatic only)
+  const float2 *twx, *twy;          // [mx], [my] exp(+2 pi i t/N)
+  GkSpeciesDev sp[GK_MAX_SPECIES];
+  float dcoef[5][2][5];             // s-derivative stencil by (class+2, sign(v)<0, d+2), units 1/ds
+  float discoef[5][5];              // s-dissipation stencil (delta^4/12 on class 0)
+};
+
+// One stage-kernel launch.
+struct GkStageArgs {
+  const void *y;     // state the RHS is evaluated on
+  const void *fn;    // f_n (modes 2: y_next = f_n + c k)
+  void *acc;         // RK accumulator
+  void *out;         // y_next / rhs / f_{n+1}
+  const float2 *phi; // potential of y
+  float2 *mom;       // moment partial planes of `out` (nullptr: skip)
+  float2 *gchi;      // per-CTA scratch for real-space grad(chi) when !gchi_in_smem
+  float c, b;        // y_next = base + c*k ; acc (+)= b*k     (dt folded in)
+  int mode;          // 0: out = k; 1: acc = y + b k, out = y + c k; 2: acc += b k, out = fn + c k;
+                     // 3: out = acc + b k
+  int nwork;         // work items = nsp*nmu*ns*nchunk
+};

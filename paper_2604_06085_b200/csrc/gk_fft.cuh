@@ -1,0 +1,238 @@
+// gk_fft.cuh -- hand-written batched shared-memory FFT building blocks for the bracket kernel.
+//
+// Sizes N = 2^a * 3^b (b <= 1), 2 <= N <= 256, as two register-resident radix passes
+// N = R1 * R2 with R1, R2 in {1,2,3,4,6,8,12,16}.  Each work item is one radix-R butterfly held
+// entirely in registers (compile-time twiddles); passes exchange data through shared memory.
+//
+// Index convention (Cooley-Tukey, n = n1 + R1*n2, k = R2*k1 + k2):
+//   nat2perm<N,S>: input in natural order, output element k = R2*k1 + k2 is left at position
+//                  q = k1 + R1*k2 (in place, no transposition pass).
+//   perm2nat<N,S>: the mirror image: input in that permuted order, output in natural order.
+// The bracket only multiplies real-space fields pointwise, so the permuted order in real space is
+// harmless and the forward transform undoes it for free (any self-consistent FFT
+// convention gives the truncated convolution).  S = +1: exp(+2 pi i nk/N), S = -1: exp(-...).
+#pragma once
+#include <cuda_runtime.h>
+#include <type_traits>
+
+namespace gkfft {
+
+template <int I> using IC = std::integral_constant<int, I>;
+
+template <int B, int E, class F>
+__device__ __forceinline__ void sfor(F &&f) {
+  if constexpr (B < E) {
+    f(IC<B>{});
+    sfor<B + 1, E>(f);
+  }
+}
+
+constexpr double kPi = 3.14159265358979323846264338327950288;
+__host__ __device__ constexpr double cx_cos(double x) {  // |x| <= pi
+  double s = 1, t = 1;
+  for (int i = 1; i <= 30; ++i) { t *= -x * x / ((2.0 * i - 1) * (2.0 * i)); s += t; }
+  return s;
+}
+__host__ __device__ constexpr double cx_sin(double x) {
+  double s = x, t = x;
+  for (int i = 1; i <= 30; ++i) { t *= -x * x / ((2.0 * i) * (2.0 * i + 1)); s += t; }
+  return s;
+}
+
+__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
+__device__ __forceinline__ float2 cmul(float2 a, float2 b) {
+  return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+}
+// multiply by S*i
+template <int S> __device__ __forceinline__ float2 muli(float2 a) {
+  return S > 0 ? make_float2(-a.y, a.x) : make_float2(a.y, -a.x);
+}
+
+// a * exp(S * 2 pi i K / N), K and N compile-time
+template <int N, int K, int S> __device__ __forceinline__ float2 mulw(float2 a) {
+  constexpr int k = ((K % N) + N) % N;
+  if constexpr (k == 0) return a;
+  else if constexpr (4 * k == N) return muli<S>(a);
+  else if constexpr (2 * k == N) return make_float2(-a.x, -a.y);
+  else if constexpr (4 * k == 3 * N) return muli<-S>(a);
+  else {
+    constexpr double ang = 2.0 * kPi * (k > N / 2 ? k - N : k) / N;
+    constexpr float c = (float)cx_cos(ang);
+    constexpr float s = (float)(S * cx_sin(ang));
+    return make_float2(a.x * c - a.y * s, a.x * s + a.y * c);
+  }
+}
+
+// In-register DFT of R points, natural order in and out.
+template <int R, int S> __device__ __forceinline__ void dft(float2 (&v)[R]) {
+  if constexpr (R == 1) {
+  } else if constexpr (R == 2) {
+    float2 a = v[0], b = v[1];
+    v[0] = cadd(a, b);
+    v[1] = csub(a, b);
+  } else if constexpr (R == 3) {
+    float2 t1 = cadd(v[1], v[2]);
+    float2 t2 = make_float2(v[0].x - 0.5f * t1.x, v[0].y - 0.5f * t1.y);
+    float2 d = csub(v[1], v[2]);
+    float2 t3 = muli<S>(make_float2(0.86602540378443864676f * d.x, 0.86602540378443864676f * d.y));
+    v[0] = cadd(v[0], t1);
+    v[1] = cadd(t2, t3);
+    v[2] = csub(t2, t3);
+  } else if constexpr (R == 4) {
+    float2 s02 = cadd(v[0], v[2]), d02 = csub(v[0], v[2]);
+    float2 s13 = cadd(v[1], v[3]), d13 = muli<S>(csub(v[1], v[3]));
+    v[0] = cadd(s02, s13);
+    v[2] = csub(s02, s13);
+    v[1] = cadd(d02, d13);
+    v[3] = csub(d02, d13);
+  } else {
+    constexpr int A = (R % 4 == 0) ? 4 : ((R % 2 == 0) ? 2 : 3);
+    constexpr int B = R / A;
+    float2 t[A][B];
+    sfor<0, A>([&](auto n1c) {
+      constexpr int n1 = decltype(n1c)::value;
+      float2 u[B];
+      sfor<0, B>([&](auto n2c) {
+        constexpr int n2 = decltype(n2c)::value;
+        u[n2] = v[n1 + A * n2];
+      });
+      dft<B, S>(u);
+      sfor<0, B>([&](auto k2c) {
+        constexpr int k2 = decltype(k2c)::value;
+        t[n1][k2] = mulw<R, n1 * k2, S>(u[k2]);
+      });
+    });
+    sfor<0, B>([&](auto k2c) {
+      constexpr int k2 = decltype(k2c)::value;
+      float2 u[A];
+      sfor<0, A>([&](auto n1c) {
+        constexpr int n1 = decltype(n1c)::value;
+        u[n1] = t[n1][k2];
+      });
+      dft<A, S>(u);
+      sfor<0, A>([&](auto k1c) {
+        constexpr int k1 = decltype(k1c)::value;
+        v[B * k1 + k2] = u[k1];
+      });
+    });
+  }
+}
+
+// two-pass factorisation N = R1 * R2
+template <int N> struct Fac;
+#define GK_FAC(N_, A_, B_) \
+  template <> struct Fac<N_> { static constexpr int R1 = A_, R2 = B_; }
+GK_FAC(2, 2, 1); GK_FAC(3, 3, 1); GK_FAC(4, 4, 1); GK_FAC(6, 6, 1); GK_FAC(8, 8, 1);
+GK_FAC(12, 12, 1); GK_FAC(16, 16, 1); GK_FAC(24, 4, 6); GK_FAC(32, 4, 8); GK_FAC(48, 6, 8);
+GK_FAC(64, 8, 8); GK_FAC(96, 8, 12); GK_FAC(128, 8, 16); GK_FAC(192, 12, 16); GK_FAC(256, 16, 16);
+#undef GK_FAC
+
+// Batched transform: element e of batch b lives at base[b*bstride + e*estride].
+// tw[t] = exp(+2 pi i t/N), t < N.  All threads of the CTA must call; ends WITHOUT a barrier.
+template <int N, int S>
+__device__ __forceinline__ void nat2perm(float2 *base, int nb, int bstride, int estride,
+                                         const float2 *tw, int tid, int nthr) {
+  constexpr int R1 = Fac<N>::R1, R2 = Fac<N>::R2;
+  if constexpr (R2 > 1) {
+    for (int w = tid; w < nb * R1; w += nthr) {
+      const int b = w % nb, n1 = w / nb;
+      float2 *p = base + b * bstride + n1 * estride;
+      float2 u[R2];
+#pragma unroll
+      for (int n2 = 0; n2 < R2; ++n2) u[n2] = p[n2 * R1 * estride];
+      dft<R2, S>(u);
+#pragma unroll
+      for (int k2 = 1; k2 < R2; ++k2) {
+        float2 t = tw[n1 * k2];
+        if (S < 0) t.y = -t.y;
+        u[k2] = cmul(u[k2], t);
+      }
+#pragma unroll
+      for (int k2 = 0; k2 < R2; ++k2) p[k2 * R1 * estride] = u[k2];
+    }
+    __syncthreads();
+  }
+  for (int w = tid; w < nb * R2; w += nthr) {
+    const int b = w % nb, k2 = w / nb;
+    float2 *p = base + b * bstride + k2 * R1 * estride;
+    float2 u[R1];
+#pragma unroll
+    for (int n1 = 0; n1 < R1; ++n1) u[n1] = p[n1 * estride];
+    dft<R1, S>(u);
+#pragma unroll
+    for (int k1 = 0; k1 < R1; ++k1) p[k1 * estride] = u[k1];
+  }
+}
+
+template <int N, int S>
+__device__ __forceinline__ void perm2nat(float2 *base, int nb, int bstride, int estride,
+                                         const float2 *tw, int tid, int nthr) {
+  constexpr int R1 = Fac<N>::R1, R2 = Fac<N>::R2;
+  for (int w = tid; w < nb * R2; w += nthr) {
+    const int b = w % nb, k2 = w / nb;
+    float2 *p = base + b * bstride + k2 * R1 * estride;
+    float2 u[R1];
+#pragma unroll
+    for (int k1 = 0; k1 < R1; ++k1) u[k1] = p[k1 * estride];
+    dft<R1, S>(u);
+    if constexpr (R2 > 1) {
+#pragma unroll
+      for (int n1 = 1; n1 < R1; ++n1) {
+        float2 t = tw[n1 * k2];
+        if (S < 0) t.y = -t.y;
+        u[n1] = cmul(u[n1], t);
+      }
+    }
+#pragma unroll
+    for (int n1 = 0; n1 < R1; ++n1) p[n1 * estride] = u[n1];
+  }
+  if constexpr (R2 > 1) {
+    __syncthreads();
+    for (int w = tid; w < nb * R1; w += nthr) {
+      const int b = w % nb, n1 = w / nb;
+      float2 *p = base + b * bstride + n1 * estride;
+      float2 u[R2];
+#pragma unroll
+      for (int k2 = 0; k2 < R2; ++k2) u[k2] = p[k2 * R1 * estride];
+      dft<R2, S>(u);
+#pragma unroll
+      for (int n2 = 0; n2 < R2; ++n2) p[n2 * R1 * estride] = u[n2];
+    }
+  }
+}
+
+#define GK_FFT_SWITCH(n, CALL)                                                            \
+  switch (n) {                                                                            \
+    case 2: CALL(2); break;     case 3: CALL(3); break;     case 4: CALL(4); break;       \
+    case 6: CALL(6); break;     case 8: CALL(8); break;     case 12: CALL(12); break;     \
+    case 16: CALL(16); break;   case 24: CALL(24); break;   case 32: CALL(32); break;     \
+    case 48: CALL(48); break;   case 64: CALL(64); break;   case 96: CALL(96); break;     \
+    case 128: CALL(128); break; case 192: CALL(192); break; case 256: CALL(256); break;   \
+    default: break;                                                                       \
+  }
+
+// runtime-size dispatch
+__device__ __forceinline__ void inv_nat2perm(int n, float2 *base, int nb, int bstride, int estride,
+                                             const float2 *tw, int tid, int nthr) {
+#define GK_CALL(N_) nat2perm<N_, +1>(base, nb, bstride, estride, tw, tid, nthr)
+  GK_FFT_SWITCH(n, GK_CALL)
+#undef GK_CALL
+}
+__device__ __forceinline__ void fwd_perm2nat(int n, float2 *base, int nb, int bstride, int estride,
+                                             const float2 *tw, int tid, int nthr) {
+#define GK_CALL(N_) perm2nat<N_, -1>(base, nb, bstride, estride, tw, tid, nthr)
+  GK_FFT_SWITCH(n, GK_CALL)
+#undef GK_CALL
+}
+
+// host helper: is n a supported transform length?
+inline bool supported_len(int n) {
+  switch (n) {
+    case 2: case 3: case 4: case 6: case 8: case 12: case 16: case 24: case 32: case 48:
+    case 64: case 96: case 128: case 192: case 256: return true;
+    default: return false;
+  }
+}
+
+}  // namespace gkfft

@@ -1,0 +1,484 @@
+// gk_lib.cu -- C ABI of libgk (include/gk.h): context, table upload, launch logic.
+// Product path.  No CPU fallback: every entry point needs a CUDA device.
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "../../include/gk.h"
+#include "gk_kernels.cuh"
+#include "gk_tables.h"
+
+namespace {
+
+constexpr size_t kSmemMax = 232448;  // 227 KB opt-in dynamic shared memory per CTA on sm_100
+
+inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+template <class T> struct DevBuf {
+  T *p = nullptr;
+  ~DevBuf() { if (p) cudaFree(p); }
+};
+
+}  // namespace
+
+struct gk_ctx {
+  gk_grid grid;
+  gk_salpha geo;
+  gk_opts opts;
+  std::vector<gk_species> species;
+  gkt::Tables T;
+  GkDev P;
+  cudaStream_t stream = nullptr;
+  std::vector<void *> dev_allocs;
+  std::string err;
+  bool poisoned = false;
+  int num_sms = 0;
+  int stage_grid = 0;
+  size_t stage_smem = 0;
+  size_t elem_bytes = 8;
+  // workspace
+  void *ws = nullptr;
+  size_t ws_bytes = 0;
+  size_t off_mom = 0, off_phi = 0, off_gchi = 0, off_ya = 0, off_yb = 0, off_acc = 0;
+  size_t need_rhs = 0, need_full = 0;
+  bool mom_valid_for_f = false;  // inside gk_rk4_steps only
+  long long launches = 0;
+  // profiling of the stage kernel
+  bool profiling = false;
+  std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ev;
+  size_t ev_used = 0;
+};
+
+namespace {
+
+int fail(gk_ctx *c, int code, const std::string &msg) {
+  if (c) {
+    c->err = msg;
+    if (code == GK_ECUDA) c->poisoned = true;
+  }
+  return code;
+}
+
+#define GK_CUDA(ctx, call)                                                                   \
+  do {                                                                                       \
+    cudaError_t e_ = (call);                                                                 \
+    if (e_ != cudaSuccess)                                                                   \
+      return fail(ctx, GK_ECUDA, std::string(#call) + ": " + cudaGetErrorString(e_));        \
+  } while (0)
+
+template <class T>
+int upload(gk_ctx *c, const std::vector<double> &src, const T **dst) {
+  std::vector<T> tmp(src.size());
+  for (size_t i = 0; i < src.size(); ++i) tmp[i] = (T)src[i];
+  void *p = nullptr;
+  cudaError_t e = cudaMalloc(&p, std::max<size_t>(tmp.size(), 1) * sizeof(T));
+  if (e != cudaSuccess) return fail(c, e == cudaErrorMemoryAllocation ? GK_ENOMEM : GK_ECUDA,
+                                    std::string("cudaMalloc(table): ") + cudaGetErrorString(e));
+  c->dev_allocs.push_back(p);
+  GK_CUDA(c, cudaMemcpy(p, tmp.data(), tmp.size() * sizeof(T), cudaMemcpyHostToDevice));
+  *dst = (const T *)p;
+  return GK_OK;
+}
+
+int smallest_pad(int nmin) {  // smallest supported 2^a 3^b (b<=1) length >= nmin
+  static const int sizes[] = {2, 3, 4, 6, 8, 12, 16, 24, 32, 48, 64, 96, 128, 192, 256};
+  for (int s : sizes)
+    if (s >= nmin) return s;
+  return -1;
+}
+
+template <class ST> void launch_moment(gk_ctx *c, const void *f, float2 *mom) {
+  const GkDev &P = c->P;
+  const int nblk_slab = (int)((P.slab + 255) / 256);
+  const long long nwork = (long long)P.nsp * P.nmu * P.nchunk * P.ns;
+  gk::gk_moment_kernel<ST><<<(unsigned)(nwork * nblk_slab), 256, 0, c->stream>>>(P, f, mom);
+  ++c->launches;
+}
+
+template <class ST> cudaError_t set_stage_attr(size_t smem, bool nl) {
+  if (nl)
+    return cudaFuncSetAttribute(gk::gk_stage_kernel<ST, true>,
+                                cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  return cudaFuncSetAttribute(gk::gk_stage_kernel<ST, false>,
+                              cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+}
+
+template <class ST> void launch_stage(gk_ctx *c, const GkStageArgs &A, bool nl) {
+  if (nl)
+    gk::gk_stage_kernel<ST, true><<<c->stage_grid, GK_STAGE_THREADS, c->stage_smem, c->stream>>>(c->P, A);
+  else
+    gk::gk_stage_kernel<ST, false><<<c->stage_grid, GK_STAGE_THREADS, c->stage_smem, c->stream>>>(c->P, A);
+  ++c->launches;
+}
+
+template <class ST> void launch_flux(gk_ctx *c, const void *f, const float2 *phi, double *out) {
+  dim3 grid((unsigned)std::min<long long>(4096, (c->P.ntot / c->P.nsp + 255) / 256), c->P.nsp);
+  gk::gk_flux_kernel<ST><<<grid, 256, 0, c->stream>>>(c->P, f, phi, out);
+  ++c->launches;
+}
+
+#define GK_BY_STORAGE(ctx, CALL)                         \
+  do {                                                   \
+    if ((ctx)->opts.storage == 0) { CALL(float2); }      \
+    else if ((ctx)->opts.storage == 1) { CALL(__half2); } \
+    else { CALL(__nv_bfloat162); }                       \
+  } while (0)
+
+int check_launch(gk_ctx *c, const char *what) {
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(c, GK_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
+  return GK_OK;
+}
+
+void stage_launch(gk_ctx *c, const GkStageArgs &A) {
+  const bool nl = (c->P.mask & GK_T_III) != 0;
+  const bool prof = c->profiling;
+  if (prof) {
+    if (c->ev_used == c->ev.size()) {
+      cudaEvent_t a, b;
+      cudaEventCreate(&a);
+      cudaEventCreate(&b);
+      c->ev.push_back({a, b});
+    }
+    cudaEventRecord(c->ev[c->ev_used].first, c->stream);
+  }
+#define GK_CALL(ST) launch_stage<ST>(c, A, nl)
+  GK_BY_STORAGE(c, GK_CALL);
+#undef GK_CALL
+  if (prof) {
+    cudaEventRecord(c->ev[c->ev_used].second, c->stream);
+    ++c->ev_used;
+  }
+}
+
+int solve_phi_from_planes(gk_ctx *c, float2 *mom, float2 *phi) {
+  const GkDev &P = c->P;
+  gk::gk_phi_kernel<<<(unsigned)((P.nphi + 255) / 256), 256, 0, c->stream>>>(P, mom, phi);
+  ++c->launches;
+  if (P.adiabatic) {
+    gk::gk_zonal_kernel<<<P.nkx, 32, 0, c->stream>>>(P, phi);
+    ++c->launches;
+  }
+  return check_launch(c, "field solve");
+}
+
+int usable(gk_ctx *c) {
+  if (!c) return GK_EINVAL;
+  if (c->poisoned) return GK_ECUDA;
+  return GK_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *gk_version(void) { return "gk-b200 0.1 (sm_100a)"; }
+
+const char *gk_last_error(const gk_ctx *c) { return c ? c->err.c_str() : "null context"; }
+
+int gk_create(const gk_grid *g, const gk_species *sp, const gk_salpha *geo, const gk_opts *o,
+              void *cuda_stream, gk_ctx **out) {
+  if (!g || !sp || !geo || !o || !out) return GK_EINVAL;
+  *out = nullptr;
+  if (g->nkx < 1 || g->nkx % 2 == 0 || g->ns < 4 || g->nvpar < 4 || g->nky < 1 || g->nmu < 1 ||
+      g->ikxspace < 1 || o->nspecies < 1 || o->nspecies > GK_MAX_SPECIES || o->storage < 0 ||
+      o->storage > 2 || !(g->vpar_max > 0) || (g->mu_grid != 0 && g->mu_grid != 1))
+    return GK_EINVAL;
+  for (int a = 0; a < o->nspecies; ++a)
+    if (sp[a].Z == 0 || !(sp[a].mass > 0) || !(sp[a].temp > 0)) return GK_EINVAL;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return GK_ECUDA;  // no CPU fallback
+
+  gk_ctx *c = new (std::nothrow) gk_ctx();
+  if (!c) return GK_ENOMEM;
+  *out = c;  // returned even on failure so that gk_last_error() can be read; caller destroys it
+  c->grid = *g; c->geo = *geo; c->opts = *o;
+  c->species.assign(sp, sp + o->nspecies);
+  c->stream = (cudaStream_t)cuda_stream;
+  c->elem_bytes = (o->storage == 0) ? 8 : 4;
+  int dev = 0;
+  GK_CUDA(c, cudaGetDevice(&dev));
+  GK_CUDA(c, cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, dev));
+
+  gkt::build_tables(*g, sp, *geo, *o, c->T);
+  const gkt::Tables &T = c->T;
+  GkDev &P = c->P;
+  std::memset(&P, 0, sizeof(P));
+  P.nsp = T.nsp; P.nv = T.nv; P.nmu = T.nmu; P.ns = T.ns; P.nkx = T.nkx; P.nky = T.nky; P.K = T.K;
+  P.ikx = g->ikxspace;
+  P.adiabatic = o->adiabatic_electrons ? 1 : 0;
+  P.mask = (o->term_mask <= 0) ? GK_T_ALL : o->term_mask;
+  if (!o->nonlinear) P.mask &= ~GK_T_III;
+  P.storage = o->storage;
+  P.ds_inv = (float)(1.0 / T.ds); P.dv_inv = (float)(1.0 / T.dv);
+  P.nu_s = (float)o->disp_par; P.nu_v = (float)o->disp_vp;
+  P.ae = o->adiabatic_electrons ? (float)(o->ne / o->te) : 0.f;
+  P.slab = (long long)T.nkx * T.nky;
+  P.nphi = (long long)T.ns * P.slab;
+  P.ntot = (long long)T.nsp * T.nv * T.nmu * P.nphi;
+  if (P.slab > (long long)GK_STAGE_THREADS * GK_EPT_MAX)
+    return fail(c, GK_EUNSUPPORTED, "nkx*nky exceeds the per-CTA slab capacity (8192)");
+  for (int a = 0; a < T.nsp; ++a) {
+    GkSpeciesDev &S = P.sp[a];
+    S.Z = (float)sp[a].Z; S.T = (float)sp[a].temp; S.mass = (float)sp[a].mass; S.dens = (float)sp[a].dens;
+    S.vR = (float)T.vR[a]; S.rlt = (float)sp[a].rlt; S.rln = (float)sp[a].rln;
+    S.ToverZ = (float)(sp[a].temp / sp[a].Z); S.ZoverT = (float)(sp[a].Z / sp[a].temp);
+    S.momfac = (float)(sp[a].Z * sp[a].dens * 2.0 * gkt::kPi * T.wv);
+  }
+  for (int q = 0; q < 50; ++q) (&P.dcoef[0][0][0])[q] = (float)(&T.dcoef[0][0][0])[q];
+  for (int q = 0; q < 25; ++q) (&P.discoef[0][0])[q] = (float)(&T.discoef[0][0])[q];
+
+  // padded grid of the bracket (3/2 rule; R14)
+  const int need_x = 3 * T.K + 1, need_y = 3 * (T.nky - 1) + 1;
+  P.mx = o->pad_mx > 0 ? o->pad_mx : smallest_pad(std::max(need_x, 2));
+  P.my = o->pad_my > 0 ? o->pad_my : smallest_pad(std::max(need_y, 2));
+  const bool nl = (P.mask & GK_T_III) != 0;
+  if (nl) {
+    if (P.mx < need_x || P.my < need_y || !gkfft::supported_len(P.mx) || !gkfft::supported_len(P.my))
+      return fail(c, GK_EUNSUPPORTED, "padded grid must be 2^a*3^b (b<=1), <=256 and satisfy the 3/2 rule");
+    if (P.mx % 2) return fail(c, GK_EUNSUPPORTED, "padded x size must be even (row pairs)");
+  }
+  P.fftnorm = (float)(1.0 / ((double)P.mx * P.my));
+  P.ldx = 2 * T.nky;
+  P.ldy = P.my | 1;
+
+  // work decomposition of the stage kernel
+  int occ_grid = c->num_sms;
+  {
+    const long long ali = (long long)T.nsp * T.nmu * T.ns;
+    long long nchunk = (6LL * occ_grid + ali - 1) / ali;
+    nchunk = std::max<long long>(1, std::min<long long>(nchunk, T.nv / 4));
+    P.jchunk = (int)((T.nv + nchunk - 1) / nchunk);
+    P.nchunk = (T.nv + P.jchunk - 1) / P.jchunk;
+    P.nparts = T.nsp * T.nmu * P.nchunk;
+  }
+  const long long nwork = (long long)T.nsp * T.nmu * T.ns * P.nchunk;
+
+  // shared-memory plan
+  if (nl) {
+    const size_t fixed = ((size_t)P.mx + P.my + (size_t)P.mx * P.ldx) * 8;
+    const size_t gbytes = (size_t)P.mx * P.ldy * 8;
+    int rc_best = 0, in_smem = 0;
+    for (int pass = 0; pass < 2 && !rc_best; ++pass) {
+      const size_t base = fixed + (pass == 0 ? gbytes : 0);
+      for (int rc = P.mx; rc >= 2; rc /= 2) {
+        if (P.mx % rc || rc % 2) continue;
+        if (base + (size_t)rc * P.ldy * 8 <= kSmemMax) {
+          // keep at least 16 rows per chunk while grad(chi) is resident, otherwise spill it
+          if (pass == 0 && rc < std::min(16, P.mx)) break;
+          rc_best = rc;
+          in_smem = (pass == 0);
+          break;
+        }
+      }
+    }
+    if (!rc_best) return fail(c, GK_EUNSUPPORTED, "padded grid does not fit the shared-memory strategy");
+    P.rc = rc_best;
+    P.gchi_in_smem = in_smem;
+    c->stage_smem = fixed + (in_smem ? gbytes : 0) + (size_t)P.rc * P.ldy * 8;
+    c->stage_grid = (int)std::min<long long>(nwork, c->num_sms);
+  } else {
+    P.rc = 2;
+    P.gchi_in_smem = 1;
+    c->stage_smem = (size_t)P.slab * 8;
+    c->stage_grid = (int)std::min<long long>(nwork, 2LL * c->num_sms);
+  }
+  {
+    cudaError_t e;
+#define GK_CALL(ST) e = set_stage_attr<ST>(c->stage_smem, nl)
+    GK_BY_STORAGE(c, GK_CALL);
+#undef GK_CALL
+    if (e != cudaSuccess) return fail(c, GK_ECUDA, std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e));
+  }
+
+  // tables -> device
+  int rcode;
+#define UP(T_, field, vec) if ((rcode = upload<T_>(c, vec, &P.field)) != GK_OK) return rcode
+  UP(float, v, T.v); UP(float, fmv, T.fmv); UP(float, mu, T.mu); UP(float, wmu, T.wmu);
+  UP(float, fmm, T.fmm); UP(float, B, T.B); UP(float, F, T.F); UP(float, BG, T.BG);
+  UP(float, sth, T.sth); UP(float, cz, T.cz); UP(float, Rmaj, T.Rmaj); UP(float, kx, T.kx);
+  UP(float, ky, T.ky); UP(float, hypx, T.hypx); UP(float, hypy, T.hypy); UP(float, J0, T.J0);
+  UP(float, dinv, T.dinv); UP(float, zinv, T.zinv);
+#undef UP
+  for (int dir = 0; dir < 2; ++dir) {
+    const int n = dir ? P.my : P.mx;
+    std::vector<float2> tw(n);
+    for (int t = 0; t < n; ++t)
+      tw[t] = make_float2((float)std::cos(2.0 * gkt::kPi * t / n), (float)std::sin(2.0 * gkt::kPi * t / n));
+    void *p = nullptr;
+    GK_CUDA(c, cudaMalloc(&p, n * sizeof(float2)));
+    c->dev_allocs.push_back(p);
+    GK_CUDA(c, cudaMemcpy(p, tw.data(), n * sizeof(float2), cudaMemcpyHostToDevice));
+    (dir ? P.twy : P.twx) = (const float2 *)p;
+  }
+
+  // workspace layout
+  size_t off = 0;
+  c->off_mom = off; off += align256((size_t)P.nparts * P.nphi * 8);
+  c->off_phi = off; off += align256((size_t)P.nphi * 8);
+  c->off_gchi = off;
+  if (nl && !P.gchi_in_smem) off += align256((size_t)c->stage_grid * P.mx * P.ldy * 8);
+  c->need_rhs = off;
+  c->off_ya = off; off += align256((size_t)P.ntot * c->elem_bytes);
+  c->off_yb = off; off += align256((size_t)P.ntot * c->elem_bytes);
+  c->off_acc = off; off += align256((size_t)P.ntot * c->elem_bytes);
+  c->need_full = off;
+  return GK_OK;
+}
+
+int gk_destroy(gk_ctx *c) {
+  if (!c) return GK_EINVAL;
+  for (void *p : c->dev_allocs) cudaFree(p);
+  for (auto &e : c->ev) { cudaEventDestroy(e.first); cudaEventDestroy(e.second); }
+  delete c;
+  return GK_OK;
+}
+
+size_t gk_workspace_bytes(const gk_ctx *c) { return c ? c->need_full : 0; }
+size_t gk_workspace_bytes_rhs(const gk_ctx *c) { return c ? c->need_rhs : 0; }
+
+int gk_set_workspace(gk_ctx *c, void *dev, size_t bytes) {
+  if (int r = usable(c)) return r;
+  if (!dev || ((uintptr_t)dev & 255) || bytes < c->need_rhs) return fail(c, GK_EINVAL, "workspace null, misaligned or too small");
+  c->ws = dev;
+  c->ws_bytes = bytes;
+  return GK_OK;
+}
+
+int gk_field_solve(gk_ctx *c, const void *f, void *phi) {
+  if (int r = usable(c)) return r;
+  if (!f || !phi || !c->ws) return fail(c, GK_EINVAL, "gk_field_solve: null pointer or no workspace");
+  float2 *mom = (float2 *)((char *)c->ws + c->off_mom);
+#define GK_CALL(ST) launch_moment<ST>(c, f, mom)
+  GK_BY_STORAGE(c, GK_CALL);
+#undef GK_CALL
+  return solve_phi_from_planes(c, mom, (float2 *)phi);
+}
+
+int gk_rhs(gk_ctx *c, const void *f, void *phi, void *rhs) {
+  if (int r = usable(c)) return r;
+  if (!f || !phi || !rhs || rhs == f || !c->ws) return fail(c, GK_EINVAL, "gk_rhs: bad pointers or no workspace");
+  if (int r = gk_field_solve(c, f, phi)) return r;
+  GkStageArgs A;
+  std::memset(&A, 0, sizeof(A));
+  A.y = f; A.out = rhs; A.phi = (const float2 *)phi; A.mode = 0;
+  A.gchi = (float2 *)((char *)c->ws + c->off_gchi);
+  A.nwork = c->P.nsp * c->P.nmu * c->P.ns * c->P.nchunk;
+  stage_launch(c, A);
+  return check_launch(c, "stage kernel");
+}
+
+int gk_rk4_steps(gk_ctx *c, void *f, double dt, int nsteps) {
+  if (int r = usable(c)) return r;
+  if (!f || !c->ws || nsteps < 0) return fail(c, GK_EINVAL, "gk_rk4_steps: bad arguments or no workspace");
+  if (c->ws_bytes < c->need_full) return fail(c, GK_EINVAL, "workspace too small for gk_rk4_step");
+  char *ws = (char *)c->ws;
+  float2 *mom = (float2 *)(ws + c->off_mom);
+  float2 *phi = (float2 *)(ws + c->off_phi);
+  void *ya = ws + c->off_ya, *yb = ws + c->off_yb, *acc = ws + c->off_acc;
+  GkStageArgs A;
+  std::memset(&A, 0, sizeof(A));
+  A.phi = phi; A.mom = mom; A.acc = acc;
+  A.gchi = (float2 *)(ws + c->off_gchi);
+  A.nwork = c->P.nsp * c->P.nmu * c->P.ns * c->P.nchunk;
+  const float h = (float)dt;
+  for (int s = 0; s < nsteps; ++s) {
+    if (s == 0) {  // later steps reuse the moment planes written by the previous stage 4
+#define GK_CALL(ST) launch_moment<ST>(c, f, mom)
+      GK_BY_STORAGE(c, GK_CALL);
+#undef GK_CALL
+    }
+    // classical RK4: acc = f + dt/6 k1, then += dt/3 k2, += dt/3 k3, f = acc + dt/6 k4
+    if (int r = solve_phi_from_planes(c, mom, phi)) return r;
+    A.mode = 1; A.y = f; A.fn = f; A.out = ya; A.c = 0.5f * h; A.b = h / 6.f;
+    stage_launch(c, A);
+    if (int r = solve_phi_from_planes(c, mom, phi)) return r;
+    A.mode = 2; A.y = ya; A.fn = f; A.out = yb; A.c = 0.5f * h; A.b = h / 3.f;
+    stage_launch(c, A);
+    if (int r = solve_phi_from_planes(c, mom, phi)) return r;
+    A.mode = 2; A.y = yb; A.fn = f; A.out = ya; A.c = h; A.b = h / 3.f;
+    stage_launch(c, A);
+    if (int r = solve_phi_from_planes(c, mom, phi)) return r;
+    A.mode = 3; A.y = ya; A.fn = f; A.out = f; A.c = 0.f; A.b = h / 6.f;
+    stage_launch(c, A);
+    if (int r = check_launch(c, "stage kernel")) return r;
+  }
+  return GK_OK;
+}
+
+int gk_rk4_step(gk_ctx *c, void *f, double dt) { return gk_rk4_steps(c, f, dt, 1); }
+
+int gk_fluxes(gk_ctx *c, const void *f, const void *phi, double *out_host) {
+  if (int r = usable(c)) return r;
+  if (!f || !phi || !out_host) return fail(c, GK_EINVAL, "gk_fluxes: null pointer");
+  double *d = nullptr;
+  GK_CUDA(c, cudaMalloc(&d, 3 * c->P.nsp * sizeof(double)));
+  cudaMemsetAsync(d, 0, 3 * c->P.nsp * sizeof(double), c->stream);
+#define GK_CALL(ST) launch_flux<ST>(c, f, (const float2 *)phi, d)
+  GK_BY_STORAGE(c, GK_CALL);
+#undef GK_CALL
+  cudaError_t e = cudaMemcpyAsync(out_host, d, 3 * c->P.nsp * sizeof(double), cudaMemcpyDeviceToHost, c->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+  cudaFree(d);
+  if (e != cudaSuccess) return fail(c, GK_ECUDA, std::string("gk_fluxes: ") + cudaGetErrorString(e));
+  // species factors: -(1/ns) 2 pi w_v  x {1, T_a, m_a vR_a}
+  for (int a = 0; a < c->P.nsp; ++a) {
+    const double base = 2.0 * gkt::kPi * c->T.wv / c->T.ns;
+    out_host[3 * a + 0] *= base;
+    out_host[3 * a + 1] *= base * c->species[a].temp;
+    out_host[3 * a + 2] *= base * c->species[a].mass * c->T.vR[a];
+  }
+  return GK_OK;
+}
+
+size_t gk_export_table(const gk_ctx *c, const char *which, double *out, size_t maxn) {
+  if (!c || !which) return 0;
+  const gkt::Tables &T = c->T;
+  const std::string w(which);
+  std::vector<double> tmp;
+  const std::vector<double> *src = nullptr;
+  if (w == "vpar") src = &T.v; else if (w == "mu") src = &T.mu; else if (w == "wmu") src = &T.wmu;
+  else if (w == "kx") src = &T.kx; else if (w == "ky") src = &T.ky; else if (w == "B") src = &T.B;
+  else if (w == "F") src = &T.F; else if (w == "BG") src = &T.BG; else if (w == "J0") src = &T.J0;
+  else if (w == "Gamma0") src = &T.G0; else if (w == "den") src = &T.den; else if (w == "zonal") src = &T.zinv;
+  else if (w == "FM") {
+    tmp.resize((size_t)T.nv * T.nmu * T.ns);
+    for (int j = 0; j < T.nv; ++j)
+      for (int l = 0; l < T.nmu; ++l)
+        for (int i = 0; i < T.ns; ++i)
+          tmp[((size_t)j * T.nmu + l) * T.ns + i] = T.fmv[j] * T.fmm[(size_t)l * T.ns + i];
+    src = &tmp;
+  } else if (w == "pad") {
+    tmp = {(double)c->P.mx, (double)c->P.my, (double)c->P.rc, (double)c->P.gchi_in_smem,
+           (double)c->P.jchunk, (double)c->P.nchunk, (double)c->stage_grid, (double)c->stage_smem};
+    src = &tmp;
+  } else return 0;
+  if (out) std::memcpy(out, src->data(), std::min(maxn, src->size()) * sizeof(double));
+  return src->size();
+}
+
+long long gk_launch_count(const gk_ctx *c) { return c ? c->launches : 0; }
+
+int gk_set_profiling(gk_ctx *c, int on) {
+  if (int r = usable(c)) return r;
+  c->profiling = on != 0;
+  return GK_OK;
+}
+
+int gk_stage_kernel_time(gk_ctx *c, double *ms_total, long long *n, int reset) {
+  if (int r = usable(c)) return r;
+  GK_CUDA(c, cudaStreamSynchronize(c->stream));
+  double tot = 0;
+  for (size_t q = 0; q < c->ev_used; ++q) {
+    float ms = 0;
+    GK_CUDA(c, cudaEventElapsedTime(&ms, c->ev[q].first, c->ev[q].second));
+    tot += ms;
+  }
+  if (ms_total) *ms_total = tot;
+  if (n) *n = (long long)c->ev_used;
+  if (reset) c->ev_used = 0;
+  return GK_OK;
+}
+
+}  // extern "C"

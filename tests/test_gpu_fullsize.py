@@ -1,0 +1,83 @@
+"""GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times: the
+oracle computes sampled (species, vpar, mu, s) slabs one by one; phi is compared in full."""
+import numpy as np
+import pytest
+
+import gkinputs
+from oracle.gkref import GkRef
+from tests.util import rel_l2
+
+pytestmark = pytest.mark.gpu
+
+
+def _sample_slabs(shape, n, seed):
+    rng = np.random.default_rng(seed)
+    nsp, nv, nmu, ns = shape[:4]
+    picks = {(0, 0, 0, 0), (nsp - 1, nv - 1, nmu - 1, ns - 1), (0, 1, 0, ns - 2), (nsp - 1, nv - 2, nmu - 1, 1)}
+    while len(picks) < n:
+        picks.add((int(rng.integers(nsp)), int(rng.integers(nv)), int(rng.integers(nmu)), int(rng.integers(ns))))
+    return sorted(picks)
+
+
+@pytest.mark.parametrize("n", [2, 3, 4, 5])
+def test_rhs_sampled_slabs_full_size(n):
+    import torch
+    from paper_2604_06085_b200 import GkContext
+    cfg = gkinputs.config(n)
+    if n == 5:
+        cfg["opts"]["storage"] = 0          # the complex64 leg of config 5
+    f = gkinputs.initial_f(cfg, np.complex64)
+    # scale so the bracket is not negligible next to the linear terms in the whole-RHS norm
+    f *= 100.0
+    g = GkContext(cfg, full_workspace=False)
+    fd = g.to_state(f)
+    rhs, phi = g.gk_rhs(fd)
+    torch.cuda.synchronize()
+    o = GkRef(cfg)
+    f128 = f.astype(np.complex128)
+    phiref = o.field_solve(f128)
+    assert rel_l2(phi.cpu().numpy(), phiref) < 1e-5
+    worst = 0.0
+    for (a, j, l, i) in _sample_slabs(o.shape, 12, 100 + n):
+        ref = o.rhs_slab(f128, phiref, a, j, l, i)
+        got = rhs[a, j, l, i].cpu().numpy()
+        worst = max(worst, rel_l2(got, ref))
+    assert worst < 1e-5, worst
+
+
+def test_config2_two_steps_full_grid():
+    from paper_2604_06085_b200 import GkContext
+    cfg = gkinputs.config(2)
+    f = gkinputs.initial_f(cfg, np.complex64)
+    g, o = GkContext(cfg), GkRef(cfg)
+    fd = g.to_state(f)
+    g.gk_rk4_steps(fd, cfg["dt"], 2)
+    ref = o.rk4_step(f, cfg["dt"], 2)
+    assert rel_l2(g.from_state(fd), ref) < 1e-4
+    assert np.isfinite(g.from_state(fd)).all()
+
+
+def test_config5_half_storage_against_complex64_run():
+    # BASELINE config 5: f stored complex fp16 vs the same run with complex64 storage (R19).
+    # 3 steps at full size; sampled slabs against the oracle would need the oracle to step the
+    # 266M-point grid, so the reference here is the complex64 GPU run (itself oracle-checked above).
+    import torch
+    from paper_2604_06085_b200 import GkContext
+    cfg32 = gkinputs.config(5)
+    cfg32["opts"]["storage"] = 0
+    cfg16 = gkinputs.config(5)
+    cfg16["opts"]["storage"] = 1
+    f = 30.0 * gkinputs.initial_f(cfg32, np.complex64)
+    g16 = GkContext(cfg16)
+    fd16 = g16.to_state(f)
+    f_rounded = g16.from_state(fd16)
+    g16.gk_rk4_steps(fd16, cfg16["dt"], 3)
+    out16 = g16.from_state(fd16)
+    del g16, fd16
+    torch.cuda.empty_cache()
+    g32 = GkContext(cfg32)
+    fd32 = g32.to_state(f_rounded)
+    g32.gk_rk4_steps(fd32, cfg32["dt"], 3)
+    out32 = g32.from_state(fd32)
+    assert np.isfinite(out16).all()
+    assert rel_l2(out16, out32) < 1e-2

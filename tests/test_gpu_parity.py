@@ -1,0 +1,188 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element on
+the same seeded inputs.  Tolerances (BASELINE.json north_star): <= 1e-5 relative L2 per gk_rhs,
+<= 1e-4 after 10 gk_rk4_step (fp32 arithmetic, complex64 storage), <= 1e-2 for half storage."""
+import numpy as np
+import pytest
+
+import gkinputs
+from oracle import gkref as G
+from oracle.gkref import GkRef
+from tests.util import small_cfg, rand_c, rel_l2
+
+pytestmark = pytest.mark.gpu
+
+TOL_RHS = 1e-5
+TOL_RK10 = 1e-4
+TOL_HALF = 1e-2
+
+
+def _ctx(cfg, **kw):
+    from paper_2604_06085_b200 import GkContext
+    return GkContext(cfg, **kw)
+
+
+MID = dict(nkx=21, nky=6, ns=8, nvpar=9, nmu=3, ikxspace=2, mu_grid=1, ky0=0.15)   # ragged sizes
+MID2 = dict(nkx=37, nky=13, ns=6, nvpar=7, nmu=2, ikxspace=3, mu_grid=1, ky0=0.05)  # 64x48 padded grid
+
+
+def test_create_time_tables_match_the_oracles():
+    cfg = small_cfg(nspecies=2, adiabatic=0, **MID)
+    g, o = _ctx(cfg), GkRef(cfg)
+    for name in ("vpar", "mu", "wmu", "kx", "ky", "B", "F", "BG", "J0", "Gamma0", "FM"):
+        np.testing.assert_allclose(g.gk_export_table(name), o.table(name).ravel(), rtol=1e-10, atol=1e-13,
+                                   err_msg=name)
+    cfg1 = gkinputs.config(1)   # Gauss-Laguerre grid
+    g, o = _ctx(cfg1), GkRef(cfg1)
+    for name in ("mu", "wmu", "J0"):
+        np.testing.assert_allclose(g.gk_export_table(name), o.table(name).ravel(), rtol=1e-10, atol=1e-13)
+    np.testing.assert_allclose(g.gk_export_table("den"), (o.table("Apol") + 1.0).ravel(), rtol=1e-12)
+
+
+@pytest.mark.parametrize("case", ["cfg1", "mid_adiabatic", "mid_kinetic", "nky1"])
+def test_field_solve_parity(case):
+    cfg = {"cfg1": gkinputs.config(1), "mid_adiabatic": small_cfg(**MID),
+           "mid_kinetic": small_cfg(nspecies=2, adiabatic=0, **MID),
+           "nky1": small_cfg(nkx=5, nky=1, ns=4, nvpar=4, nmu=1)}[case]
+    g, o = _ctx(cfg), GkRef(cfg)
+    f = rand_c(np.random.default_rng(31), o.shape, True).astype(np.complex64)
+    phi = g.gk_field_solve(g.to_state(f)).cpu().numpy()
+    ref = o.field_solve(f)
+    assert rel_l2(phi, ref) < TOL_RHS
+    K = (cfg["grid"]["nkx"] - 1) // 2
+    assert np.all(phi[:, K, 0] == 0)
+
+
+@pytest.mark.parametrize("bit", range(10))
+def test_rhs_parity_one_term_at_a_time(bit):
+    # every term separately, relative to ITS OWN norm (the bracket is tiny next to the linear terms
+    # at amplitude 1e-3 and would hide inside a whole-RHS norm)
+    cfg = small_cfg(**MID)
+    mask = 1 << bit
+    g, o = _ctx(cfg, term_mask=mask), GkRef(cfg, term_mask=mask, bracket_method=1)
+    f = rand_c(np.random.default_rng(32), o.shape, False).astype(np.complex64)   # asymmetric ky=0
+    rhs, phi = g.gk_rhs(g.to_state(f))
+    ref, _ = o.rhs(f)
+    assert np.linalg.norm(ref) > 0
+    assert rel_l2(rhs.cpu().numpy(), ref) < TOL_RHS, bit
+
+
+@pytest.mark.parametrize("case", ["cfg1", "mid", "mid2", "mid_kinetic", "closure1", "tiny"])
+def test_rhs_parity_full(case):
+    cfg = {"cfg1": gkinputs.config(1), "mid": small_cfg(**MID), "mid2": small_cfg(**MID2),
+           "mid_kinetic": small_cfg(nspecies=2, adiabatic=0, **MID),
+           "closure1": small_cfg(s_closure=1, **MID),
+           "tiny": small_cfg(nkx=3, nky=2, ns=4, nvpar=4, nmu=1)}[case]
+    g, o = _ctx(cfg), GkRef(cfg)
+    f = gkinputs.initial_f(cfg, np.complex64) if case == "cfg1" else \
+        rand_c(np.random.default_rng(33), o.shape, True).astype(np.complex64)
+    rhs, phi = g.gk_rhs(g.to_state(f))
+    ref, phiref = o.rhs(f)
+    assert rel_l2(phi.cpu().numpy(), phiref) < TOL_RHS
+    assert rel_l2(rhs.cpu().numpy(), ref) < TOL_RHS
+
+
+def test_bracket_independent_of_padded_size_and_matches_direct_convolution():
+    cfg = small_cfg(**MID)     # K=10 -> 31, nky=6 -> 16: minimal supported 32 x 16
+    o = GkRef(cfg, term_mask=G.T_III, bracket_method=1)
+    f = rand_c(np.random.default_rng(34), o.shape, True).astype(np.complex64)
+    ref, _ = o.rhs(f)
+    for pad in [(32, 16), (48, 24), (64, 32), (32, 48)]:
+        g = _ctx(cfg, term_mask=G.T_III, pad=pad)
+        assert g.plan()["mx"] == pad[0] and g.plan()["my"] == pad[1]
+        rhs, _ = g.gk_rhs(g.to_state(f))
+        assert rel_l2(rhs.cpu().numpy(), ref) < TOL_RHS, pad
+
+
+def test_bracket_antisymmetry_on_device():
+    # sum_k P_m Re[conj(f_k) III_k] = 0 per slab (free-energy conservation of the nonlinearity)
+    cfg = small_cfg(**MID)
+    g = _ctx(cfg, term_mask=G.T_III)
+    f = rand_c(np.random.default_rng(35), GkRef(cfg).shape, True).astype(np.complex64)
+    rhs = g.gk_rhs(g.to_state(f))[0].cpu().numpy().astype(np.complex128)
+    P = np.where(np.arange(6) == 0, 1.0, 2.0)
+    num = (P * (np.conj(f) * rhs).real).sum(axis=(-1, -2))
+    den = (P * abs(f) * abs(rhs)).sum(axis=(-1, -2))
+    assert (abs(num) / den).max() < 2e-6
+
+
+@pytest.mark.parametrize("case", ["cfg1", "mid"])
+def test_rk4_ten_steps_parity(case):
+    cfg = gkinputs.config(1) if case == "cfg1" else small_cfg(**MID)
+    g, o = _ctx(cfg), GkRef(cfg)
+    f = gkinputs.initial_f(cfg, np.complex64)
+    dt = cfg["dt"]
+    fd = g.to_state(f)
+    for _ in range(10):
+        g.gk_rk4_step(fd, dt)
+    ref = o.rk4_step(f, dt, 10)
+    assert rel_l2(g.from_state(fd), ref) < TOL_RK10
+    # the multi-step entry point (moments carried between steps) gives the same trajectory
+    fd2 = g.to_state(f)
+    g.gk_rk4_steps(fd2, dt, 10)
+    assert rel_l2(g.from_state(fd2), g.from_state(fd)) < 1e-6
+
+
+def test_rk4_large_amplitude_nonlinear_step():
+    # amplitude O(1): the bracket is as large as the linear terms
+    cfg = small_cfg(**MID)
+    g, o = _ctx(cfg), GkRef(cfg)
+    f = rand_c(np.random.default_rng(36), o.shape, True).astype(np.complex64)
+    fd = g.to_state(f)
+    g.gk_rk4_steps(fd, 0.005, 2)
+    ref = o.rk4_step(f, 0.005, 2)
+    assert rel_l2(g.from_state(fd), ref) < TOL_RK10
+
+
+@pytest.mark.parametrize("storage", [1, 2])
+def test_half_storage_variant(storage):
+    # BASELINE config 5 variant (R19): f, stage states and accumulator in complex fp16/bf16,
+    # arithmetic fp32.  fp16 is compared after 10 steps, bf16 (8-bit mantissa) after 3.
+    cfg = small_cfg(storage=storage, **MID)
+    g = _ctx(cfg)
+    o = GkRef(small_cfg(**MID))
+    f = 30.0 * gkinputs.initial_f(cfg, np.complex64)       # 0.03: inside fp16's normal range
+    fd = g.to_state(f)
+    fq = g.from_state(fd)                                   # the rounded initial state
+    rhs, _ = g.gk_rhs(fd)
+    ref, _ = o.rhs(fq)
+    assert rel_l2(g.from_state(rhs), ref) < TOL_HALF
+    n = 10 if storage == 1 else 3
+    g.gk_rk4_steps(fd, cfg["dt"], n)
+    assert rel_l2(g.from_state(fd), o.rk4_step(fq, cfg["dt"], n)) < TOL_HALF
+
+
+def test_fluxes_parity_and_particle_flux_invariant():
+    cfg = small_cfg(**MID)
+    g, o = _ctx(cfg), GkRef(cfg)
+    f = rand_c(np.random.default_rng(37), o.shape, True).astype(np.complex64)
+    fd = g.to_state(f)
+    phi = g.gk_field_solve(fd)
+    fl = g.gk_fluxes(fd, phi)
+    ref = o.fluxes(f, o.field_solve(f))
+    np.testing.assert_allclose(fl[:, 1:], ref[:, 1:], rtol=2e-4)
+    assert abs(fl[0, 0]) < 1e-4 * abs(fl[0, 1])
+    cfgk = small_cfg(nspecies=2, adiabatic=0, **MID)
+    g, o = _ctx(cfgk), GkRef(cfgk)
+    f = rand_c(np.random.default_rng(38), o.shape, True).astype(np.complex64)
+    fd = g.to_state(f)
+    np.testing.assert_allclose(g.gk_fluxes(fd, g.gk_field_solve(fd)), o.fluxes(f, o.field_solve(f)), rtol=5e-4)
+
+
+def test_error_behaviour():
+    from paper_2604_06085_b200 import GkError
+    from paper_2604_06085_b200 import binding as b
+    import ctypes as C
+    with pytest.raises(GkError) as ei:
+        _ctx(small_cfg(nkx=8))
+    assert ei.value.code == b.GK_EINVAL
+    with pytest.raises(GkError) as ei:
+        _ctx(small_cfg(**MID), pad=(16, 16))                # violates the 3/2 rule
+    assert ei.value.code == b.GK_EUNSUPPORTED
+    g = _ctx(gkinputs.config(1), full_workspace=False)
+    fd = g.to_state(gkinputs.initial_f(gkinputs.config(1)))
+    with pytest.raises(GkError) as ei:                      # rk4 needs the full workspace
+        g.gk_rk4_step(fd, 0.01)
+    assert ei.value.code == b.GK_EINVAL
+    assert g.lib.gk_rhs(g._h, C.c_void_p(fd.data_ptr()), None, None) == b.GK_EINVAL
+    g.gk_rhs(fd)                                            # still usable after an EINVAL
+    assert g.gk_launch_count() >= 4
