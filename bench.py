@@ -1,0 +1,285 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the gyrokinetic RK stage (field solve -> linear terms -> ExB bracket
+-> RK4 stage update) on synthetic seeded grids shaped like the paper's workloads.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl gk|reference]
+
+A "step" is one classical RK4 step = 4 passes of the whole hot path over the 5-D grid.
+metric = 5-D grid-point RK-stage updates per second = points * 4 * steps / time.
+N > 1 (torchrun): the paper has no grid parallelism -> independent replicas, one per
+GPU, no data-path collective ("scaling": "weak").  Prints ONE JSON line on rank 0.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+import gkinputs  # noqa: E402
+
+METRIC = "5D grid-point RK-stage updates/s"
+UNIT = "stage-updates/s"
+# algorithmic HBM bytes per grid point per stage launch: classical RK4 with the
+# accumulator initialised in stage 1: stages move 24, 40, 40, 24 B/pt (complex64) -> 32 on average
+ALG_BYTES_PER_POINT_STAGE = {0: 32.0, 1: 16.0, 2: 16.0}
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as fh:
+            d = json.load(fh)
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def _traffic(workload):
+    p = os.path.join(ROOT, "profiles", "stage_traffic.json")
+    if os.path.exists(p):
+        with open(p) as fh:
+            return json.load(fh).get(workload)
+    return None
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm = [float(r[0]) for r in self.rows if r and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) > 1 and r[1].replace(".", "").isdigit()]
+        reasons = set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            for k, n in enumerate(names):
+                if len(r) > 3 + k and r[3 + k].lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def _oracle_sample(cfg, budget_s=15.0):
+    """The oracle as it stands on the host cores, bounded sample: one full field solve plus as many
+    whole (species,vpar,mu,s) slabs of gk_rhs as fit in the budget, slabs spread over `cores`
+    threads (the oracle's own rhs loop is the same slab loop under OpenMP)."""
+    from concurrent.futures import ThreadPoolExecutor
+
+    from oracle import gkref
+    cores = os.cpu_count() or 1
+    gkref.set_threads(cores)
+    o = gkref.GkRef(cfg)
+    f = gkinputs.initial_f(cfg, np.complex128)
+    t0 = time.perf_counter()
+    phi = o.field_solve(f)
+    t_field = time.perf_counter() - t0
+    nsp, nv, nmu, ns, nkx, nky = o.shape
+    nslabs = nsp * nv * nmu * ns
+    rng = np.random.default_rng(7)
+    picks = [(int(rng.integers(nsp)), int(rng.integers(nv)), int(rng.integers(nmu)), int(rng.integers(ns)))
+             for _ in range(nslabs)]
+    done, t1 = 0, time.perf_counter()
+    batch = cores * 4
+    with ThreadPoolExecutor(cores) as ex:
+        while done < nslabs and time.perf_counter() - t1 < budget_s:
+            list(ex.map(lambda q: o.rhs_slab(f, phi, *q), picks[done:done + batch]))
+            done += batch
+    t_slabs = time.perf_counter() - t1
+    done = min(done, nslabs)
+    est_stage = t_field + t_slabs * nslabs / done
+    n = int(np.prod(o.shape))
+    return {"value": n / est_stage, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"full field solve ({t_field:.2f}s) + {done} of {nslabs} slabs of gk_rhs "
+                      f"({t_slabs:.1f}s) on {cores} threads, extrapolated to one stage"}
+
+
+def run_reference(args, cfg, rank):
+    if rank != 0:
+        return
+    per_step = max(2.0, min(20.0, 100.0 / max(args.steps + args.warmup, 1)))
+    vals = []
+    for s in range(args.warmup + args.steps):
+        r = _oracle_sample(cfg, budget_s=per_step)
+        if s >= args.warmup:
+            vals.append(r)
+    v = float(np.mean([r["value"] for r in vals]))
+    n = int(np.prod(gkinputs.f_shape(cfg)))
+    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * 4 * n / v,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": {"workload": cfg["name"], "note": "CPU oracle, bounded sample per step"},
+            "cpu_baseline": {**vals[-1], "value": v},
+            "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json config number 1..5")
+    ap.add_argument("--impl", default="gk", choices=["gk", "reference"])
+    ap.add_argument("--storage", type=int, default=None, help="override storage (0 c64, 1 fp16, 2 bf16)")
+    ap.add_argument("--linear", action="store_true", help="switch term III off (HBM-bound variant)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs)")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "gk" else args.warmup
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    cfg = gkinputs.config(args.config)
+    if args.storage is not None:
+        cfg["opts"]["storage"] = args.storage
+    if args.linear:
+        cfg["opts"]["nonlinear"] = 0
+    if args.impl == "reference":
+        run_reference(args, cfg, rank)
+        return
+
+    import torch
+    import torch.distributed as dist
+    from paper_2604_06085_b200 import GkContext
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device and no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    cfg["seed"] += rank                     # replicas differ only in their seed
+    g = GkContext(cfg, device=dev)
+    f_host = gkinputs.initial_f(cfg, np.complex64)
+    fd = g.to_state(f_host)
+    npts = int(np.prod(g.shape))
+    dt = cfg["dt"]
+    storage = g.storage
+
+    # ---- device-resident throughput ----
+    g.gk_rk4_steps(fd, dt, args.warmup)
+    barrier()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    g.gk_set_profiling(True)
+    g.gk_stage_kernel_time(reset=True)
+    l0 = g.gk_launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    g.gk_rk4_steps(fd, dt, args.steps)
+    e1.record()
+    barrier()
+    ms = e0.elapsed_time(e1)
+    launches = g.gk_launch_count() - l0
+    stage_ms, stage_n = g.gk_stage_kernel_time(reset=True)
+    g.gk_set_profiling(False)
+    clocks = sampler.stop()
+    finite = bool(torch.isfinite(torch.view_as_real(fd) if storage == 0 else fd.float()).all().item())
+    t = torch.tensor([ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_max = float(t.item())
+    value = world * npts * 4 * args.steps / (ms_max * 1e-3)
+
+    # ---- end to end: host buffers, H2D of f and D2H of f_{n+1} inside the timed region ----
+    e2e_steps = max(1, min(args.steps, 5))
+    if args.no_e2e:
+        e2e_steps = 0
+    hbuf = torch.empty(fd.shape if e2e_steps else (1,), dtype=fd.dtype).pin_memory()
+    if e2e_steps:
+        hbuf.copy_(fd.cpu())
+    for _ in range(2 if e2e_steps else 0):
+        fd.copy_(hbuf, non_blocking=True)
+        g.gk_rk4_step(fd, dt)
+        hbuf.copy_(fd, non_blocking=True)
+    barrier()
+    e0.record()
+    for _ in range(e2e_steps):
+        fd.copy_(hbuf, non_blocking=True)
+        g.gk_rk4_step(fd, dt)
+        hbuf.copy_(fd, non_blocking=True)
+    e1.record()
+    barrier()
+    t = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    e2e_value = world * npts * 4 * e2e_steps / (float(t.item()) * 1e-3) if e2e_steps else None
+    fbytes = fd.numel() * fd.element_size()
+
+    if rank == 0:
+        peak, peak_src = _peaks()
+        bpp = ALG_BYTES_PER_POINT_STAGE[storage]
+        stage_avg_ms = stage_ms / max(stage_n, 1)
+        achieved = bpp * npts / (stage_avg_ms * 1e-3) / 1e9
+        plan = g.plan()
+        nl = bool(cfg["opts"]["nonlinear"])
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None,
+            "dtype": {0: "f32", 1: "f32 (fp16 storage)", 2: "f32 (bf16 storage)"}[storage],
+            "data": "synthetic",
+            "config": {"workload": cfg["name"], "grid": cfg["grid"], "nspecies": g.nsp, "points": npts,
+                       "nonlinear": nl, "dt": dt, "padded_fft": [plan["mx"], plan["my"]],
+                       "l2": "inputs larger than L2 (state + 3 work arrays)" if npts * 8 * 4 > 126e6 * 2
+                       else "working set comparable to L2; not flushed",
+                       "parallelism": "replicas only (paper has no grid parallelism)", "finite": finite},
+            "clocks": clocks,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": fbytes, "d2h_bytes_per_step": fbytes,
+                    "steps": e2e_steps},
+            "gpu_launches": int(launches),
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                         "frac": achieved / peak, "traffic": _traffic(cfg["name"]), "peak_source": peak_src,
+                         "kernel": "gk_stage_kernel", "launches_timed": int(stage_n),
+                         "avg_launch_ms": stage_avg_ms, "alg_bytes_per_point": bpp,
+                         "stage_share_of_step": stage_ms / ms if ms > 0 else None},
+        }
+        if not args.no_cpu_baseline and world == 1:
+            line["cpu_baseline"] = _oracle_sample(cfg, budget_s=12.0)
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()
