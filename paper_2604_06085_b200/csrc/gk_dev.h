@@ -24,6 +24,9 @@ struct GkDev {
   int nparts;          // number of moment partial planes = nsp*nmu*nchunk
   int gchi_in_smem;    // 1: real-space grad(chi) lives in shared memory, 0: per-CTA global scratch
   float ds_inv, dv_inv;
+  float dkx, ky0;      // kx_p = p*dkx, ky_m = m*ky0
+  float invK, invM;    // 1/K, 1/(nky-1) (0 if degenerate)
+  float hyp_x, hyp_y;  // nu_x, nu_y of the hyper-viscosity (0 if masked off)
   float nu_s, nu_v;
   float ae;            // ne/Te of the adiabatic electrons
   float fftnorm;       // 1/(mx*my)
@@ -55,6 +58,7 @@ struct GkStageArgs {
   const float2 *phi; // potential of y
   float2 *mom;       // moment partial planes of `out` (nullptr: skip)
   float2 *gchi;      // per-CTA scratch for real-space grad(chi) when !gchi_in_smem
+  float2 *chis;      // per-CTA scratch, 3*slab: chi = J0 phi, D_s chi for v>0, D_s chi for v<0
   float c, b;        // y_next = base + c*k ; acc (+)= b*k     (dt folded in)
   int mode;          // 0: out = k; 1: acc = y + b k, out = y + c k; 2: acc += b k, out = fn + c k;
                      // 3: out = acc + b k

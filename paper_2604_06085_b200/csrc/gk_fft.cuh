@@ -202,6 +202,54 @@ __device__ __forceinline__ void perm2nat(float2 *base, int nb, int bstride, int 
   }
 }
 
+// Same as nat2perm, but the natural-order input of batch b, index n comes from LOAD(b, n) (global
+// memory, or another shared array combined on the fly) instead of the destination array: the
+// first radix pass doubles as the load/zero-pad/pre-multiply pass.
+template <int N, int S, class LOAD>
+__device__ __forceinline__ void nat2perm_load(float2 *base, int nb, int bstride, int estride,
+                                              const float2 *tw, int tid, int nthr, LOAD load) {
+  constexpr int R1 = Fac<N>::R1, R2 = Fac<N>::R2;
+  if constexpr (R2 > 1) {
+    for (int w = tid; w < nb * R1; w += nthr) {
+      const int b = w % nb, n1 = w / nb;
+      float2 *p = base + b * bstride + n1 * estride;
+      float2 u[R2];
+#pragma unroll
+      for (int n2 = 0; n2 < R2; ++n2) u[n2] = load(b, n1 + R1 * n2);
+      dft<R2, S>(u);
+#pragma unroll
+      for (int k2 = 1; k2 < R2; ++k2) {
+        float2 t = tw[n1 * k2];
+        if (S < 0) t.y = -t.y;
+        u[k2] = cmul(u[k2], t);
+      }
+#pragma unroll
+      for (int k2 = 0; k2 < R2; ++k2) p[k2 * R1 * estride] = u[k2];
+    }
+    __syncthreads();
+    for (int w = tid; w < nb * R2; w += nthr) {
+      const int b = w % nb, k2 = w / nb;
+      float2 *p = base + b * bstride + k2 * R1 * estride;
+      float2 u[R1];
+#pragma unroll
+      for (int n1 = 0; n1 < R1; ++n1) u[n1] = p[n1 * estride];
+      dft<R1, S>(u);
+#pragma unroll
+      for (int k1 = 0; k1 < R1; ++k1) p[k1 * estride] = u[k1];
+    }
+  } else {
+    for (int b = tid; b < nb; b += nthr) {
+      float2 *p = base + b * bstride;
+      float2 u[R1];
+#pragma unroll
+      for (int n1 = 0; n1 < R1; ++n1) u[n1] = load(b, n1);
+      dft<R1, S>(u);
+#pragma unroll
+      for (int k1 = 0; k1 < R1; ++k1) p[k1 * estride] = u[k1];
+    }
+  }
+}
+
 #define GK_FFT_SWITCH(n, CALL)                                                            \
   switch (n) {                                                                            \
     case 2: CALL(2); break;     case 3: CALL(3); break;     case 4: CALL(4); break;       \
@@ -212,18 +260,28 @@ __device__ __forceinline__ void perm2nat(float2 *base, int nb, int bstride, int 
     default: break;                                                                       \
   }
 
-// runtime-size dispatch
-__device__ __forceinline__ void inv_nat2perm(int n, float2 *base, int nb, int bstride, int estride,
-                                             const float2 *tw, int tid, int nthr) {
-#define GK_CALL(N_) nat2perm<N_, +1>(base, nb, bstride, estride, tw, tid, nthr)
-  GK_FFT_SWITCH(n, GK_CALL)
+// Size dispatch: NC > 0 is a compile-time length (specialised kernels), NC == 0 switches on n.
+template <int NC, class LOAD>
+__device__ __forceinline__ void inv_nat2perm_load(int n, float2 *base, int nb, int bstride, int estride,
+                                                  const float2 *tw, int tid, int nthr, LOAD load) {
+  if constexpr (NC > 0) {
+    nat2perm_load<NC, +1>(base, nb, bstride, estride, tw, tid, nthr, load);
+  } else {
+#define GK_CALL(N_) nat2perm_load<N_, +1>(base, nb, bstride, estride, tw, tid, nthr, load)
+    GK_FFT_SWITCH(n, GK_CALL)
 #undef GK_CALL
+  }
 }
+template <int NC>
 __device__ __forceinline__ void fwd_perm2nat(int n, float2 *base, int nb, int bstride, int estride,
                                              const float2 *tw, int tid, int nthr) {
+  if constexpr (NC > 0) {
+    perm2nat<NC, -1>(base, nb, bstride, estride, tw, tid, nthr);
+  } else {
 #define GK_CALL(N_) perm2nat<N_, -1>(base, nb, bstride, estride, tw, tid, nthr)
-  GK_FFT_SWITCH(n, GK_CALL)
+    GK_FFT_SWITCH(n, GK_CALL)
 #undef GK_CALL
+  }
 }
 
 // host helper: is n a supported transform length?

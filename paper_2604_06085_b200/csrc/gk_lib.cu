@@ -40,7 +40,8 @@ struct gk_ctx {
   // workspace
   void *ws = nullptr;
   size_t ws_bytes = 0;
-  size_t off_mom = 0, off_phi = 0, off_gchi = 0, off_ya = 0, off_yb = 0, off_acc = 0;
+  size_t off_mom = 0, off_phi = 0, off_gchi = 0, off_chis = 0, off_ya = 0, off_yb = 0, off_acc = 0;
+  const void *stage_fn = nullptr;  // the gk_stage_kernel instantiation chosen at create time
   size_t need_rhs = 0, need_full = 0;
   bool mom_valid_for_f = false;  // inside gk_rk4_steps only
   long long launches = 0;
@@ -96,19 +97,23 @@ template <class ST> void launch_moment(gk_ctx *c, const void *f, float2 *mom) {
   ++c->launches;
 }
 
-template <class ST> cudaError_t set_stage_attr(size_t smem, bool nl) {
-  if (nl)
-    return cudaFuncSetAttribute(gk::gk_stage_kernel<ST, true>,
-                                cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  return cudaFuncSetAttribute(gk::gk_stage_kernel<ST, false>,
-                              cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+// Stage-kernel instantiations: the four BASELINE shapes get compile-time sizes (index arithmetic and
+// FFT radices fold to constants); everything else runs the generic kernel.
+template <class ST> const void *pick_stage(int mx, int my, int nky, int nkx, bool nl) {
+  if (!nl) return (const void *)gk::gk_stage_kernel<ST, 0, 0, 0, 0, false>;
+#define GK_SPEC(MX, MY, NKY, NKX) \
+  if (mx == MX && my == MY && nky == NKY && nkx == NKX) return (const void *)gk::gk_stage_kernel<ST, MX, MY, NKY, NKX, true>
+  GK_SPEC(16, 12, 4, 9);
+  GK_SPEC(128, 48, 16, 85);
+  GK_SPEC(128, 96, 32, 85);
+  GK_SPEC(192, 192, 64, 127);
+#undef GK_SPEC
+  return (const void *)gk::gk_stage_kernel<ST, 0, 0, 0, 0, true>;
 }
 
-template <class ST> void launch_stage(gk_ctx *c, const GkStageArgs &A, bool nl) {
-  if (nl)
-    gk::gk_stage_kernel<ST, true><<<c->stage_grid, GK_STAGE_THREADS, c->stage_smem, c->stream>>>(c->P, A);
-  else
-    gk::gk_stage_kernel<ST, false><<<c->stage_grid, GK_STAGE_THREADS, c->stage_smem, c->stream>>>(c->P, A);
+void launch_stage(gk_ctx *c, const GkStageArgs &A) {
+  void *args[2] = {(void *)&c->P, (void *)&A};
+  cudaLaunchKernel(c->stage_fn, dim3(c->stage_grid), dim3(GK_STAGE_THREADS), args, c->stage_smem, c->stream);
   ++c->launches;
 }
 
@@ -132,7 +137,6 @@ int check_launch(gk_ctx *c, const char *what) {
 }
 
 void stage_launch(gk_ctx *c, const GkStageArgs &A) {
-  const bool nl = (c->P.mask & GK_T_III) != 0;
   const bool prof = c->profiling;
   if (prof) {
     if (c->ev_used == c->ev.size()) {
@@ -143,9 +147,7 @@ void stage_launch(gk_ctx *c, const GkStageArgs &A) {
     }
     cudaEventRecord(c->ev[c->ev_used].first, c->stream);
   }
-#define GK_CALL(ST) launch_stage<ST>(c, A, nl)
-  GK_BY_STORAGE(c, GK_CALL);
-#undef GK_CALL
+  launch_stage(c, A);
   if (prof) {
     cudaEventRecord(c->ev[c->ev_used].second, c->stream);
     ++c->ev_used;
@@ -210,9 +212,14 @@ int gk_create(const gk_grid *g, const gk_species *sp, const gk_salpha *geo, cons
   P.adiabatic = o->adiabatic_electrons ? 1 : 0;
   P.mask = (o->term_mask <= 0) ? GK_T_ALL : o->term_mask;
   if (!o->nonlinear) P.mask &= ~GK_T_III;
+  P.hyp_x = (P.mask & GK_T_HYP) ? (float)o->disp_x : 0.f;
+  P.hyp_y = (P.mask & GK_T_HYP) ? (float)o->disp_y : 0.f;
   P.storage = o->storage;
   P.ds_inv = (float)(1.0 / T.ds); P.dv_inv = (float)(1.0 / T.dv);
   P.nu_s = (float)o->disp_par; P.nu_v = (float)o->disp_vp;
+  P.dkx = (float)T.dkx; P.ky0 = (float)g->ky0;
+  P.invK = T.K > 0 ? (float)(1.0 / T.K) : 0.f;
+  P.invM = T.nky > 1 ? (float)(1.0 / (T.nky - 1)) : 0.f;
   P.ae = o->adiabatic_electrons ? (float)(o->ne / o->te) : 0.f;
   P.slab = (long long)T.nkx * T.nky;
   P.nphi = (long long)T.ns * P.slab;
@@ -240,7 +247,7 @@ int gk_create(const gk_grid *g, const gk_species *sp, const gk_salpha *geo, cons
     if (P.mx % 2) return fail(c, GK_EUNSUPPORTED, "padded x size must be even (row pairs)");
   }
   P.fftnorm = (float)(1.0 / ((double)P.mx * P.my));
-  P.ldx = 2 * T.nky;
+  P.ldx = 2 * T.nky + 1;
   P.ldy = P.my | 1;
 
   // work decomposition of the stage kernel
@@ -285,10 +292,10 @@ int gk_create(const gk_grid *g, const gk_species *sp, const gk_salpha *geo, cons
     c->stage_grid = (int)std::min<long long>(nwork, 2LL * c->num_sms);
   }
   {
-    cudaError_t e;
-#define GK_CALL(ST) e = set_stage_attr<ST>(c->stage_smem, nl)
+#define GK_CALL(ST) c->stage_fn = pick_stage<ST>(P.mx, P.my, P.nky, P.nkx, nl)
     GK_BY_STORAGE(c, GK_CALL);
 #undef GK_CALL
+    cudaError_t e = cudaFuncSetAttribute(c->stage_fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->stage_smem);
     if (e != cudaSuccess) return fail(c, GK_ECUDA, std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e));
   }
 
@@ -319,6 +326,7 @@ int gk_create(const gk_grid *g, const gk_species *sp, const gk_salpha *geo, cons
   c->off_phi = off; off += align256((size_t)P.nphi * 8);
   c->off_gchi = off;
   if (nl && !P.gchi_in_smem) off += align256((size_t)c->stage_grid * P.mx * P.ldy * 8);
+  c->off_chis = off; off += align256((size_t)c->stage_grid * 3 * P.slab * 8);
   c->need_rhs = off;
   c->off_ya = off; off += align256((size_t)P.ntot * c->elem_bytes);
   c->off_yb = off; off += align256((size_t)P.ntot * c->elem_bytes);
@@ -364,6 +372,7 @@ int gk_rhs(gk_ctx *c, const void *f, void *phi, void *rhs) {
   std::memset(&A, 0, sizeof(A));
   A.y = f; A.out = rhs; A.phi = (const float2 *)phi; A.mode = 0;
   A.gchi = (float2 *)((char *)c->ws + c->off_gchi);
+  A.chis = (float2 *)((char *)c->ws + c->off_chis);
   A.nwork = c->P.nsp * c->P.nmu * c->P.ns * c->P.nchunk;
   stage_launch(c, A);
   return check_launch(c, "stage kernel");
@@ -381,6 +390,7 @@ int gk_rk4_steps(gk_ctx *c, void *f, double dt, int nsteps) {
   std::memset(&A, 0, sizeof(A));
   A.phi = phi; A.mom = mom; A.acc = acc;
   A.gchi = (float2 *)(ws + c->off_gchi);
+  A.chis = (float2 *)(ws + c->off_chis);
   A.nwork = c->P.nsp * c->P.nmu * c->P.ns * c->P.nchunk;
   const float h = (float)dt;
   for (int s = 0; s < nsteps; ++s) {
