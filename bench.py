@@ -125,6 +125,34 @@ def _oracle_sample(cfg, budget_s=15.0):
                       f"({t_slabs:.1f}s) on {cores} threads, extrapolated to one stage"}
 
 
+def replica_config(config_no: int, rank: int, storage=None, linear=False) -> dict:
+    """Workload of one rank: the paper has no grid parallelism, so N GPUs run N
+    independent replicas of the same configuration that differ only in their seed."""
+    cfg = gkinputs.config(config_no)
+    if storage is not None:
+        cfg["opts"]["storage"] = storage
+    if linear:
+        cfg["opts"]["nonlinear"] = 0
+    cfg["seed"] += rank
+    return cfg
+
+
+def max_over_ranks(value: float, world: int, device=None) -> float:
+    """Timing rule of the bench contract: the slowest rank defines the step time."""
+    if world <= 1:
+        return float(value)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([value], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(npts: int, steps: int, world: int, ms_max: float) -> float:
+    """Whole-job stage-updates/s: every rank advanced npts points through 4 stages per step."""
+    return world * npts * 4 * steps / (ms_max * 1e-3)
+
+
 def run_reference(args, cfg, rank):
     if rank != 0:
         return
@@ -163,14 +191,10 @@ def main():
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
-    cfg = gkinputs.config(args.config)
-    if args.storage is not None:
-        cfg["opts"]["storage"] = args.storage
-    if args.linear:
-        cfg["opts"]["nonlinear"] = 0
     if args.impl == "reference":
-        run_reference(args, cfg, rank)
+        run_reference(args, replica_config(args.config, 0, args.storage, args.linear), rank)
         return
+    cfg = replica_config(args.config, rank, args.storage, args.linear)
 
     import torch
     import torch.distributed as dist
@@ -188,7 +212,6 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    cfg["seed"] += rank                     # replicas differ only in their seed
     g = GkContext(cfg, device=dev)
     f_host = gkinputs.initial_f(cfg, np.complex64)
     fd = g.to_state(f_host)
@@ -215,11 +238,8 @@ def main():
     g.gk_set_profiling(False)
     clocks = sampler.stop()
     finite = bool(torch.isfinite(torch.view_as_real(fd) if storage == 0 else fd.float()).all().item())
-    t = torch.tensor([ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_max = float(t.item())
-    value = world * npts * 4 * args.steps / (ms_max * 1e-3)
+    ms_max = max_over_ranks(ms, world, dev)
+    value = aggregate_value(npts, args.steps, world, ms_max)
 
     # ---- end to end: host buffers, H2D of f and D2H of f_{n+1} inside the timed region ----
     e2e_steps = max(1, min(args.steps, 5))
@@ -240,10 +260,8 @@ def main():
         hbuf.copy_(fd, non_blocking=True)
     e1.record()
     barrier()
-    t = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    e2e_value = world * npts * 4 * e2e_steps / (float(t.item()) * 1e-3) if e2e_steps else None
+    e2e_ms = max_over_ranks(e0.elapsed_time(e1), world, dev)
+    e2e_value = aggregate_value(npts, e2e_steps, world, e2e_ms) if e2e_steps else None
     fbytes = fd.numel() * fd.element_size()
 
     if rank == 0:

@@ -1,6 +1,7 @@
 // gk_lib.cu -- C ABI of libgk (include/gk.h): context, table upload, launch logic.
 // Product path.  No CPU fallback: every entry point needs a CUDA device.
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <string>
 #include <vector>
@@ -35,6 +36,7 @@ struct gk_ctx {
   bool poisoned = false;
   int num_sms = 0;
   int stage_grid = 0;
+  int stage_threads = 512, stage_occ = 1;
   size_t stage_smem = 0;
   size_t elem_bytes = 8;
   // workspace
@@ -98,22 +100,28 @@ template <class ST> void launch_moment(gk_ctx *c, const void *f, float2 *mom) {
 }
 
 // Stage-kernel instantiations: the four BASELINE shapes get compile-time sizes (index arithmetic and
-// FFT radices fold to constants); everything else runs the generic kernel.
-template <class ST> const void *pick_stage(int mx, int my, int nky, int nkx, bool nl) {
-  if (!nl) return (const void *)gk::gk_stage_kernel<ST, 0, 0, 0, 0, false>;
-#define GK_SPEC(MX, MY, NKY, NKX) \
-  if (mx == MX && my == MY && nky == NKY && nkx == NKX) return (const void *)gk::gk_stage_kernel<ST, MX, MY, NKY, NKX, true>
-  GK_SPEC(16, 12, 4, 9);
-  GK_SPEC(128, 48, 16, 85);
-  GK_SPEC(128, 96, 32, 85);
-  GK_SPEC(192, 192, 64, 127);
+// FFT radices fold to constants); everything else runs the generic kernel.  occ = 2 variants keep
+// grad(chi) in global scratch so that two 256-thread CTAs share an SM.
+struct StagePick { const void *fn; int threads; int occ; };
+template <class ST> StagePick pick_stage(int mx, int my, int nky, int nkx, bool nl, int want_occ) {
+  if (!nl) return {(const void *)gk::gk_stage_kernel<ST, 0, 0, 0, 0, false, 512, 1>, 512, 1};
+#define GK_SPEC(MX, MY, NKY, NKX, NT, OCC)                                          \
+  if (mx == MX && my == MY && nky == NKY && nkx == NKX && want_occ == OCC)          \
+    return {(const void *)gk::gk_stage_kernel<ST, MX, MY, NKY, NKX, true, NT, OCC>, NT, OCC}
+  GK_SPEC(16, 12, 4, 9, 512, 1);
+  GK_SPEC(128, 48, 16, 85, 512, 1);
+  GK_SPEC(128, 48, 16, 85, 256, 2);
+  GK_SPEC(128, 96, 32, 85, 512, 1);
+  GK_SPEC(128, 96, 32, 85, 256, 2);
+  GK_SPEC(192, 192, 64, 127, 512, 1);
 #undef GK_SPEC
-  return (const void *)gk::gk_stage_kernel<ST, 0, 0, 0, 0, true>;
+  if (want_occ != 1) return pick_stage<ST>(mx, my, nky, nkx, nl, 1);
+  return {(const void *)gk::gk_stage_kernel<ST, 0, 0, 0, 0, true, 512, 1>, 512, 1};
 }
 
 void launch_stage(gk_ctx *c, const GkStageArgs &A) {
   void *args[2] = {(void *)&c->P, (void *)&A};
-  cudaLaunchKernel(c->stage_fn, dim3(c->stage_grid), dim3(GK_STAGE_THREADS), args, c->stage_smem, c->stream);
+  cudaLaunchKernel(c->stage_fn, dim3(c->stage_grid), dim3(c->stage_threads), args, c->stage_smem, c->stream);
   ++c->launches;
 }
 
@@ -224,7 +232,7 @@ int gk_create(const gk_grid *g, const gk_species *sp, const gk_salpha *geo, cons
   P.slab = (long long)T.nkx * T.nky;
   P.nphi = (long long)T.ns * P.slab;
   P.ntot = (long long)T.nsp * T.nv * T.nmu * P.nphi;
-  if (P.slab > (long long)GK_STAGE_THREADS * GK_EPT_MAX)
+  if (P.slab > (long long)GK_SLAB_MAX)
     return fail(c, GK_EUNSUPPORTED, "nkx*nky exceeds the per-CTA slab capacity (8192)");
   for (int a = 0; a < T.nsp; ++a) {
     GkSpeciesDev &S = P.sp[a];
@@ -250,51 +258,67 @@ int gk_create(const gk_grid *g, const gk_species *sp, const gk_salpha *geo, cons
   P.ldx = 2 * T.nky + 1;
   P.ldy = P.my | 1;
 
-  // work decomposition of the stage kernel
-  int occ_grid = c->num_sms;
-  {
-    const long long ali = (long long)T.nsp * T.nmu * T.ns;
-    long long nchunk = (6LL * occ_grid + ali - 1) / ali;
-    nchunk = std::max<long long>(1, std::min<long long>(nchunk, T.nv / 4));
-    P.jchunk = (int)((T.nv + nchunk - 1) / nchunk);
-    P.nchunk = (T.nv + P.jchunk - 1) / P.jchunk;
-    P.nparts = T.nsp * T.nmu * P.nchunk;
-  }
-  const long long nwork = (long long)T.nsp * T.nmu * T.ns * P.nchunk;
-
-  // shared-memory plan
-  if (nl) {
-    const size_t fixed = ((size_t)P.mx + P.my + (size_t)P.mx * P.ldx) * 8;
-    const size_t gbytes = (size_t)P.mx * P.ldy * 8;
-    int rc_best = 0, in_smem = 0;
-    for (int pass = 0; pass < 2 && !rc_best; ++pass) {
-      const size_t base = fixed + (pass == 0 ? gbytes : 0);
-      for (int rc = P.mx; rc >= 2; rc /= 2) {
-        if (P.mx % rc || rc % 2) continue;
-        if (base + (size_t)rc * P.ldy * 8 <= kSmemMax) {
-          // keep at least 16 rows per chunk while grad(chi) is resident, otherwise spill it
-          if (pass == 0 && rc < std::min(16, P.mx)) break;
-          rc_best = rc;
-          in_smem = (pass == 0);
-          break;
-        }
-      }
-    }
-    if (!rc_best) return fail(c, GK_EUNSUPPORTED, "padded grid does not fit the shared-memory strategy");
-    P.rc = rc_best;
-    P.gchi_in_smem = in_smem;
-    c->stage_smem = fixed + (in_smem ? gbytes : 0) + (size_t)P.rc * P.ldy * 8;
-    c->stage_grid = (int)std::min<long long>(nwork, c->num_sms);
-  } else {
-    P.rc = 2;
-    P.gchi_in_smem = 1;
-    c->stage_smem = (size_t)P.slab * 8;
-    c->stage_grid = (int)std::min<long long>(nwork, 2LL * c->num_sms);
-  }
-  {
-#define GK_CALL(ST) c->stage_fn = pick_stage<ST>(P.mx, P.my, P.nky, P.nkx, nl)
+  // Kernel variant.  Two CTAs per SM (256 threads each) overlap one CTA's memory-bound epilogue with
+  // the other's FFT phases, but only pay off while grad(chi) still fits in shared memory; otherwise
+  // one 512-thread CTA per SM.  GK_STAGE_OCC=1|2 overrides the choice (tuning knob).
+  int want_occ = 2;
+  if (const char *env = std::getenv("GK_STAGE_OCC")) want_occ = std::atoi(env) == 1 ? 1 : 2;
+  long long nwork = 0;
+  for (int attempt = 0; attempt < 2; ++attempt) {
+    StagePick pick;
+#define GK_CALL(ST) pick = pick_stage<ST>(P.mx, P.my, P.nky, P.nkx, nl, want_occ)
     GK_BY_STORAGE(c, GK_CALL);
 #undef GK_CALL
+    c->stage_fn = pick.fn;
+    c->stage_threads = pick.threads;
+    c->stage_occ = pick.occ;
+    const int resident = c->num_sms * pick.occ;  // persistent CTAs
+
+    // work decomposition: >= 6 work items per resident CTA, vpar chunks >= 4 long
+    {
+      const long long ali = (long long)T.nsp * T.nmu * T.ns;
+      long long nchunk = (6LL * resident + ali - 1) / ali;
+      nchunk = std::max<long long>(1, std::min<long long>(nchunk, T.nv / 4));
+      P.jchunk = (int)((T.nv + nchunk - 1) / nchunk);
+      P.nchunk = (T.nv + P.jchunk - 1) / P.jchunk;
+      P.nparts = T.nsp * T.nmu * P.nchunk;
+    }
+    nwork = (long long)T.nsp * T.nmu * T.ns * P.nchunk;
+
+    // shared-memory plan (per CTA: the SM's 227 KB opt-in capacity / occ, minus 1 KB reserved per CTA)
+    if (nl) {
+      const size_t cap = pick.occ == 1 ? kSmemMax : (kSmemMax + 1024) / pick.occ - 1024;
+      const size_t fixed = ((size_t)P.mx + P.my + (size_t)P.mx * P.ldx) * 8;
+      const size_t gbytes = (size_t)P.mx * P.ldy * 8;
+      int rc_best = 0, in_smem = 0;
+      for (int pass = 0; pass < 2 && !rc_best; ++pass) {
+        const size_t base = fixed + (pass == 0 ? gbytes : 0);
+        for (int rc = P.mx; rc >= 2; rc /= 2) {
+          if (P.mx % rc || rc % 2) continue;
+          if (base + (size_t)rc * P.ldy * 8 <= cap) {
+            // keep at least 16 rows per chunk while grad(chi) is resident, otherwise spill it
+            if (pass == 0 && rc < std::min(16, P.mx)) break;
+            rc_best = rc;
+            in_smem = (pass == 0);
+            break;
+          }
+        }
+      }
+      if (pick.occ == 2 && !in_smem && attempt == 0) { want_occ = 1; continue; }
+      if (!rc_best) return fail(c, GK_EUNSUPPORTED, "padded grid does not fit the shared-memory strategy");
+      P.rc = rc_best;
+      P.gchi_in_smem = in_smem;
+      c->stage_smem = fixed + (in_smem ? gbytes : 0) + (size_t)P.rc * P.ldy * 8;
+      c->stage_grid = (int)std::min<long long>(nwork, resident);
+    } else {
+      P.rc = 2;
+      P.gchi_in_smem = 1;
+      c->stage_smem = (size_t)P.slab * 8;
+      c->stage_grid = (int)std::min<long long>(nwork, 2LL * c->num_sms);
+    }
+    break;
+  }
+  {
     cudaError_t e = cudaFuncSetAttribute(c->stage_fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->stage_smem);
     if (e != cudaSuccess) return fail(c, GK_ECUDA, std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e));
   }
@@ -461,7 +485,8 @@ size_t gk_export_table(const gk_ctx *c, const char *which, double *out, size_t m
     src = &tmp;
   } else if (w == "pad") {
     tmp = {(double)c->P.mx, (double)c->P.my, (double)c->P.rc, (double)c->P.gchi_in_smem,
-           (double)c->P.jchunk, (double)c->P.nchunk, (double)c->stage_grid, (double)c->stage_smem};
+           (double)c->P.jchunk, (double)c->P.nchunk, (double)c->stage_grid, (double)c->stage_smem,
+           (double)c->stage_threads, (double)c->stage_occ};
     src = &tmp;
   } else return 0;
   if (out) std::memcpy(out, src->data(), std::min(maxn, src->size()) * sizeof(double));

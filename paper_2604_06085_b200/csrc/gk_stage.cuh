@@ -20,8 +20,7 @@
 
 namespace gk {
 
-#define GK_STAGE_THREADS 512
-#define GK_EPT_MAX 16  // slab elements per thread for the moment accumulators (512*16 = 8192)
+#define GK_SLAB_MAX 8192  // largest nkx*nky a CTA handles (moment accumulators live in registers)
 
 struct SlabCtx {  // quantities uniform over a slab (a, j, l, i)
   int a, j, l, i, sg;
@@ -155,12 +154,16 @@ __device__ __forceinline__ float2 rhs_point(const GkDev &P, const GkStageArgs &A
 }
 
 // =================================================================================================
-template <class ST, int MX_, int MY_, int NKY_, int NKX_, bool NL>
-__global__ void __launch_bounds__(GK_STAGE_THREADS, 1)
+// NT threads per CTA, OCC resident CTAs per SM (OCC = 2: grad(chi) is kept in the per-CTA global
+// scratch so that two CTAs fit one SM and their memory-bound and FFT phases overlap).
+template <class ST, int MX_, int MY_, int NKY_, int NKX_, bool NL, int NT, int OCC>
+__global__ void __launch_bounds__(NT, OCC)
 gk_stage_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkStageArgs A) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   constexpr bool SPEC = (MX_ > 0);
-  const int tid = threadIdx.x, nthr = GK_STAGE_THREADS;
+  const int tid = threadIdx.x;
+  constexpr int nthr = NT;
+  constexpr int EPT = SPEC ? (NKX_ * NKY_ + NT - 1) / NT : GK_SLAB_MAX / NT;
   const int mx = SPEC ? MX_ : P.mx, my = SPEC ? MY_ : P.my;
   const int nky = SPEC ? NKY_ : P.nky, nkx = SPEC ? NKX_ : P.nkx;
   const int K = (nkx - 1) / 2, slab = nkx * nky;
@@ -267,9 +270,9 @@ gk_stage_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkStage
                 });
       }
     }
-    float2 macc[GK_EPT_MAX];
+    float2 macc[EPT];
 #pragma unroll
-    for (int k = 0; k < GK_EPT_MAX; ++k) macc[k] = make_float2(0.f, 0.f);
+    for (int k = 0; k < EPT; ++k) macc[k] = make_float2(0.f, 0.f);
     const int j1 = min(P.nv, (c + 1) * P.jchunk);
     for (int j = c * P.jchunk; j < j1; ++j) {
       SlabCtx C;
@@ -341,7 +344,7 @@ gk_stage_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkStage
       }
       if (A.mom) {  // the same thread wrote these entries: no barrier needed
 #pragma unroll
-        for (int k = 0; k < GK_EPT_MAX; ++k) {
+        for (int k = 0; k < EPT; ++k) {
           const int e = tid + k * nthr;
           if (e < slab) {
             const int ip = e / nky, m = e - ip * nky;
@@ -354,7 +357,7 @@ gk_stage_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkStage
     if (A.mom) {
       float2 *dst = A.mom + (((long long)a * P.nmu + l) * P.nchunk + c) * P.nphi + (long long)i * P.slab;
 #pragma unroll
-      for (int k = 0; k < GK_EPT_MAX; ++k) {
+      for (int k = 0; k < EPT; ++k) {
         const int e = tid + k * nthr;
         if (e < slab) dst[e] = macc[k];
       }

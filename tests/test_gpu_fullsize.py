@@ -45,6 +45,22 @@ def test_rhs_sampled_slabs_full_size(n):
     assert worst < 1e-5, worst
 
 
+@pytest.mark.parametrize("n", [2, 3, 4, 5])
+def test_configured_run_stays_bounded(n):
+    # before timing, run the configured step count and assert ||f|| stays finite and
+    # grows < 10x (config 5: complex64 leg).  Configs 3-5 are run for 10 steps here.
+    import torch
+    from paper_2604_06085_b200 import GkContext
+    cfg = gkinputs.config(n)
+    cfg["opts"]["storage"] = 0
+    g = GkContext(cfg)
+    fd = g.to_state(gkinputs.initial_f(cfg, np.complex64))
+    n0 = float(torch.linalg.vector_norm(torch.view_as_real(fd)))
+    g.gk_rk4_steps(fd, cfg["dt"], cfg["steps"] if n == 2 else 10)
+    n1 = float(torch.linalg.vector_norm(torch.view_as_real(fd)))
+    assert np.isfinite(n1) and n1 < 10 * n0, (n0, n1)
+
+
 def test_config2_two_steps_full_grid():
     from paper_2604_06085_b200 import GkContext
     cfg = gkinputs.config(2)

@@ -135,6 +135,23 @@ def test_time_stepped_growth_matches_eigen_solve():
     assert np.argmax(prof) in (3, 4)
 
 
+def test_kinetic_electron_omega_h_mode_sets_the_smallest_stable_kperp():
+    # Why BASELINE config 4 runs at ky0 = 0.2 (R5): with kinetic electrons the zonal
+    # (ky=0, kx=dkx) chain carries the electrostatic omega_H mode, |lambda| ~ k_par v_te/(k_perp rho).
+    # Explicit RK4 at dt = 0.002 amplifies it when k_perp = dkx is too small (PAPER.md:356 lists this
+    # "field CFL" among the timestep limits).
+    amp = {}
+    for ky0 in (0.035, 0.2):
+        cfg = small_cfg(nkx=3, nky=1, ns=32, nvpar=8, nmu=1, nspecies=2, adiabatic=0, mu_grid=1, ky0=ky0,
+                        ikxspace=5, nonlinear=0)
+        o = GkRef(cfg)
+        sel = np.zeros(o.shape, bool)
+        sel[:, :, :, :, 2, 0] = True
+        z = np.linalg.eigvals(_operator_matrix(o, sel)) * 0.002
+        amp[ky0] = abs(1 + z + z ** 2 / 2 + z ** 3 / 6 + z ** 4 / 24).max()
+    assert amp[0.035] > 10 and amp[0.2] < 1.0, amp
+
+
 @pytest.mark.slow
 def test_rosenbluth_hinton_residual():
     # PAPER.md:134, 460-468 (eq. 5): q=1.3, eps=0.05, shat=0.1592, s-alpha, k_psi rho = 0.025,
