@@ -128,83 +128,18 @@ GK_FAC(12, 12, 1); GK_FAC(16, 16, 1); GK_FAC(24, 4, 6); GK_FAC(32, 4, 8); GK_FAC
 GK_FAC(64, 8, 8); GK_FAC(96, 8, 12); GK_FAC(128, 8, 16); GK_FAC(192, 12, 16); GK_FAC(256, 16, 16);
 #undef GK_FAC
 
-// Batched transform: element e of batch b lives at base[b*bstride + e*estride].
-// tw[t] = exp(+2 pi i t/N), t < N.  All threads of the CTA must call; ends WITHOUT a barrier.
-template <int N, int S>
-__device__ __forceinline__ void nat2perm(float2 *base, int nb, int bstride, int estride,
-                                         const float2 *tw, int tid, int nthr) {
-  constexpr int R1 = Fac<N>::R1, R2 = Fac<N>::R2;
-  if constexpr (R2 > 1) {
-    for (int w = tid; w < nb * R1; w += nthr) {
-      const int b = w % nb, n1 = w / nb;
-      float2 *p = base + b * bstride + n1 * estride;
-      float2 u[R2];
-#pragma unroll
-      for (int n2 = 0; n2 < R2; ++n2) u[n2] = p[n2 * R1 * estride];
-      dft<R2, S>(u);
-#pragma unroll
-      for (int k2 = 1; k2 < R2; ++k2) {
-        float2 t = tw[n1 * k2];
-        if (S < 0) t.y = -t.y;
-        u[k2] = cmul(u[k2], t);
-      }
-#pragma unroll
-      for (int k2 = 0; k2 < R2; ++k2) p[k2 * R1 * estride] = u[k2];
-    }
-    __syncthreads();
-  }
-  for (int w = tid; w < nb * R2; w += nthr) {
-    const int b = w % nb, k2 = w / nb;
-    float2 *p = base + b * bstride + k2 * R1 * estride;
-    float2 u[R1];
-#pragma unroll
-    for (int n1 = 0; n1 < R1; ++n1) u[n1] = p[n1 * estride];
-    dft<R1, S>(u);
-#pragma unroll
-    for (int k1 = 0; k1 < R1; ++k1) p[k1 * estride] = u[k1];
-  }
-}
-
-template <int N, int S>
-__device__ __forceinline__ void perm2nat(float2 *base, int nb, int bstride, int estride,
-                                         const float2 *tw, int tid, int nthr) {
-  constexpr int R1 = Fac<N>::R1, R2 = Fac<N>::R2;
-  for (int w = tid; w < nb * R2; w += nthr) {
-    const int b = w % nb, k2 = w / nb;
-    float2 *p = base + b * bstride + k2 * R1 * estride;
-    float2 u[R1];
-#pragma unroll
-    for (int k1 = 0; k1 < R1; ++k1) u[k1] = p[k1 * estride];
-    dft<R1, S>(u);
-    if constexpr (R2 > 1) {
-#pragma unroll
-      for (int n1 = 1; n1 < R1; ++n1) {
-        float2 t = tw[n1 * k2];
-        if (S < 0) t.y = -t.y;
-        u[n1] = cmul(u[n1], t);
-      }
-    }
-#pragma unroll
-    for (int n1 = 0; n1 < R1; ++n1) p[n1 * estride] = u[n1];
-  }
-  if constexpr (R2 > 1) {
-    __syncthreads();
-    for (int w = tid; w < nb * R1; w += nthr) {
-      const int b = w % nb, n1 = w / nb;
-      float2 *p = base + b * bstride + n1 * estride;
-      float2 u[R2];
-#pragma unroll
-      for (int k2 = 0; k2 < R2; ++k2) u[k2] = p[k2 * R1 * estride];
-      dft<R2, S>(u);
-#pragma unroll
-      for (int n2 = 0; n2 < R2; ++n2) p[n2 * R1 * estride] = u[n2];
-    }
-  }
-}
-
-// Same as nat2perm, but the natural-order input of batch b, index n comes from LOAD(b, n) (global
-// memory, or another shared array combined on the fly) instead of the destination array: the
-// first radix pass doubles as the load/zero-pad/pre-multiply pass.
+// Batched transforms: element e of batch b lives at base[b*bstride + e*estride];
+// tw[t] = exp(+2 pi i t/N), t < N.  All threads of the CTA must call; they end WITHOUT a barrier.
+//
+// Fused variants.  The natural-order side of a transform is produced / consumed by a functor that
+// receives the index split as (run-time base, compile-time offset, compile-time span):
+//     n = nbase + OFF,  0 <= nbase < SPAN
+// so a caller with compile-time sizes can decide with `if constexpr` which elements are zero
+// padding (never loaded) or not needed (never stored -> the dead arithmetic is eliminated).
+//
+// nat2perm_load:  natural-order input of batch b from LOAD(b, nbase, IC<OFF>, IC<SPAN>) (global
+//   memory, or another shared array combined on the fly): the first radix pass doubles as the
+//   load / zero-pad / pre-multiply pass.  Output digit-permuted in `base`.
 template <int N, int S, class LOAD>
 __device__ __forceinline__ void nat2perm_load(float2 *base, int nb, int bstride, int estride,
                                               const float2 *tw, int tid, int nthr, LOAD load) {
@@ -214,8 +149,10 @@ __device__ __forceinline__ void nat2perm_load(float2 *base, int nb, int bstride,
       const int b = w % nb, n1 = w / nb;
       float2 *p = base + b * bstride + n1 * estride;
       float2 u[R2];
-#pragma unroll
-      for (int n2 = 0; n2 < R2; ++n2) u[n2] = load(b, n1 + R1 * n2);
+      sfor<0, R2>([&](auto n2c) {
+        constexpr int n2 = decltype(n2c)::value;
+        u[n2] = load(b, n1, IC<R1 * n2>{}, IC<R1>{});
+      });
       dft<R2, S>(u);
 #pragma unroll
       for (int k2 = 1; k2 < R2; ++k2) {
@@ -241,11 +178,66 @@ __device__ __forceinline__ void nat2perm_load(float2 *base, int nb, int bstride,
     for (int b = tid; b < nb; b += nthr) {
       float2 *p = base + b * bstride;
       float2 u[R1];
-#pragma unroll
-      for (int n1 = 0; n1 < R1; ++n1) u[n1] = load(b, n1);
+      sfor<0, R1>([&](auto n1c) {
+        constexpr int n1 = decltype(n1c)::value;
+        u[n1] = load(b, 0, IC<n1>{}, IC<1>{});
+      });
       dft<R1, S>(u);
 #pragma unroll
       for (int k1 = 0; k1 < R1; ++k1) p[k1 * estride] = u[k1];
+    }
+  }
+}
+
+// perm2nat_fused: digit-permuted input of batch b, position q, from LOADP(b, q) (may combine
+//   several shared arrays: the pointwise bracket is evaluated here); natural-order output handed
+//   to STORE(b, nbase, IC<OFF>, IC<SPAN>, value).  `base` is the exchange buffer between the
+//   two radix passes; LOADP may read it at the positions its own work item overwrites.
+template <int N, int S, class LOADP, class STORE>
+__device__ __forceinline__ void perm2nat_fused(float2 *base, int nb, int bstride, int estride,
+                                               const float2 *tw, int tid, int nthr, LOADP loadp,
+                                               STORE store) {
+  constexpr int R1 = Fac<N>::R1, R2 = Fac<N>::R2;
+  if constexpr (R2 > 1) {
+    for (int w = tid; w < nb * R2; w += nthr) {
+      const int b = w % nb, k2 = w / nb;
+      float2 *p = base + b * bstride + k2 * R1 * estride;
+      float2 u[R1];
+#pragma unroll
+      for (int k1 = 0; k1 < R1; ++k1) u[k1] = loadp(b, k2 * R1 + k1);
+      dft<R1, S>(u);
+#pragma unroll
+      for (int n1 = 1; n1 < R1; ++n1) {
+        float2 t = tw[n1 * k2];
+        if (S < 0) t.y = -t.y;
+        u[n1] = cmul(u[n1], t);
+      }
+#pragma unroll
+      for (int n1 = 0; n1 < R1; ++n1) p[n1 * estride] = u[n1];
+    }
+    __syncthreads();
+    for (int w = tid; w < nb * R1; w += nthr) {
+      const int b = w % nb, n1 = w / nb;
+      const float2 *p = base + b * bstride + n1 * estride;
+      float2 u[R2];
+#pragma unroll
+      for (int k2 = 0; k2 < R2; ++k2) u[k2] = p[k2 * R1 * estride];
+      dft<R2, S>(u);
+      sfor<0, R2>([&](auto n2c) {
+        constexpr int n2 = decltype(n2c)::value;
+        store(b, n1, IC<R1 * n2>{}, IC<R1>{}, u[n2]);
+      });
+    }
+  } else {
+    for (int b = tid; b < nb; b += nthr) {
+      float2 u[R1];
+#pragma unroll
+      for (int k1 = 0; k1 < R1; ++k1) u[k1] = loadp(b, k1);
+      dft<R1, S>(u);
+      sfor<0, R1>([&](auto n1c) {
+        constexpr int n1 = decltype(n1c)::value;
+        store(b, 0, IC<n1>{}, IC<1>{}, u[n1]);
+      });
     }
   }
 }
@@ -272,13 +264,14 @@ __device__ __forceinline__ void inv_nat2perm_load(int n, float2 *base, int nb, i
 #undef GK_CALL
   }
 }
-template <int NC>
-__device__ __forceinline__ void fwd_perm2nat(int n, float2 *base, int nb, int bstride, int estride,
-                                             const float2 *tw, int tid, int nthr) {
+template <int NC, class LOADP, class STORE>
+__device__ __forceinline__ void fwd_perm2nat_fused(int n, float2 *base, int nb, int bstride, int estride,
+                                                   const float2 *tw, int tid, int nthr, LOADP loadp,
+                                                   STORE store) {
   if constexpr (NC > 0) {
-    perm2nat<NC, -1>(base, nb, bstride, estride, tw, tid, nthr);
+    perm2nat_fused<NC, -1>(base, nb, bstride, estride, tw, tid, nthr, loadp, store);
   } else {
-#define GK_CALL(N_) perm2nat<N_, -1>(base, nb, bstride, estride, tw, tid, nthr)
+#define GK_CALL(N_) perm2nat_fused<N_, -1>(base, nb, bstride, estride, tw, tid, nthr, loadp, store)
     GK_FFT_SWITCH(n, GK_CALL)
 #undef GK_CALL
   }

@@ -103,19 +103,30 @@ template <class ST> void launch_moment(gk_ctx *c, const void *f, float2 *mom) {
 // FFT radices fold to constants); everything else runs the generic kernel.  occ = 2 variants keep
 // grad(chi) in global scratch so that two 256-thread CTAs share an SM.
 struct StagePick { const void *fn; int threads; int occ; };
-template <class ST> StagePick pick_stage(int mx, int my, int nky, int nkx, bool nl, int want_occ) {
+template <class ST> StagePick pick_stage(int mx, int my, int nky, int nkx, bool nl, int want_occ, int want_thr) {
   if (!nl) return {(const void *)gk::gk_stage_kernel<ST, 0, 0, 0, 0, false, 512, 1>, 512, 1};
-#define GK_SPEC(MX, MY, NKY, NKX, NT, OCC)                                          \
-  if (mx == MX && my == MY && nky == NKY && nkx == NKX && want_occ == OCC)          \
+#define GK_SPEC(MX, MY, NKY, NKX, NT, OCC)                                                       \
+  if (mx == MX && my == MY && nky == NKY && nkx == NKX && want_occ == OCC && want_thr == NT)     \
     return {(const void *)gk::gk_stage_kernel<ST, MX, MY, NKY, NKX, true, NT, OCC>, NT, OCC}
   GK_SPEC(16, 12, 4, 9, 512, 1);
-  GK_SPEC(128, 48, 16, 85, 512, 1);
-  GK_SPEC(128, 48, 16, 85, 256, 2);
+  GK_SPEC(128, 48, 16, 85, 1024, 1);
+  GK_SPEC(128, 48, 16, 85, 512, 2);
+  GK_SPEC(128, 96, 32, 85, 1024, 1);
   GK_SPEC(128, 96, 32, 85, 512, 1);
-  GK_SPEC(128, 96, 32, 85, 256, 2);
+  GK_SPEC(192, 192, 64, 127, 1024, 1);
   GK_SPEC(192, 192, 64, 127, 512, 1);
 #undef GK_SPEC
-  if (want_occ != 1) return pick_stage<ST>(mx, my, nky, nkx, nl, 1);
+  return {nullptr, 0, 0};
+}
+// preference order of (threads, occ) variants; the first one that exists and fits is used
+template <class ST> StagePick pick_stage_auto(int mx, int my, int nky, int nkx, bool nl, int force_occ, int force_thr) {
+  static const int pref[][2] = {{1024, 1}, {512, 2}, {512, 1}};
+  for (auto &pr : pref) {
+    if (force_thr && pr[0] != force_thr) continue;
+    if (force_occ && pr[1] != force_occ) continue;
+    StagePick p = pick_stage<ST>(mx, my, nky, nkx, nl, pr[1], pr[0]);
+    if (p.fn) return p;
+  }
   return {(const void *)gk::gk_stage_kernel<ST, 0, 0, 0, 0, true, 512, 1>, 512, 1};
 }
 
@@ -131,12 +142,16 @@ template <class ST> void launch_flux(gk_ctx *c, const void *f, const float2 *phi
   ++c->launches;
 }
 
+#ifdef GK_ONLY_C64  // developer builds (GK_FAST_BUILD=1): complex64 storage only, 3x faster to compile
+#define GK_BY_STORAGE(ctx, CALL) do { CALL(float2); } while (0)
+#else
 #define GK_BY_STORAGE(ctx, CALL)                         \
   do {                                                   \
     if ((ctx)->opts.storage == 0) { CALL(float2); }      \
     else if ((ctx)->opts.storage == 1) { CALL(__half2); } \
     else { CALL(__nv_bfloat162); }                       \
   } while (0)
+#endif
 
 int check_launch(gk_ctx *c, const char *what) {
   cudaError_t e = cudaGetLastError();
@@ -197,6 +212,9 @@ int gk_create(const gk_grid *g, const gk_species *sp, const gk_salpha *geo, cons
     return GK_EINVAL;
   for (int a = 0; a < o->nspecies; ++a)
     if (sp[a].Z == 0 || !(sp[a].mass > 0) || !(sp[a].temp > 0)) return GK_EINVAL;
+#ifdef GK_ONLY_C64
+  if (o->storage != 0) return GK_EUNSUPPORTED;
+#endif
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return GK_ECUDA;  // no CPU fallback
 
@@ -258,15 +276,16 @@ int gk_create(const gk_grid *g, const gk_species *sp, const gk_salpha *geo, cons
   P.ldx = 2 * T.nky + 1;
   P.ldy = P.my | 1;
 
-  // Kernel variant.  Two CTAs per SM (256 threads each) overlap one CTA's memory-bound epilogue with
-  // the other's FFT phases, but only pay off while grad(chi) still fits in shared memory; otherwise
-  // one 512-thread CTA per SM.  GK_STAGE_OCC=1|2 overrides the choice (tuning knob).
-  int want_occ = 2;
-  if (const char *env = std::getenv("GK_STAGE_OCC")) want_occ = std::atoi(env) == 1 ? 1 : 2;
+  // Kernel variant: (threads per CTA, CTAs per SM) by measured preference; GK_STAGE_THREADS and
+  // GK_STAGE_OCC override the choice (tuning knobs).  A variant whose shared-memory plan needs
+  // grad(chi) spilled to global scratch at occ = 2 is skipped in favour of one CTA per SM.
+  int force_occ = 0, force_thr = 0;
+  if (const char *env = std::getenv("GK_STAGE_OCC")) force_occ = std::atoi(env);
+  if (const char *env = std::getenv("GK_STAGE_THREADS")) force_thr = std::atoi(env);
   long long nwork = 0;
   for (int attempt = 0; attempt < 2; ++attempt) {
     StagePick pick;
-#define GK_CALL(ST) pick = pick_stage<ST>(P.mx, P.my, P.nky, P.nkx, nl, want_occ)
+#define GK_CALL(ST) pick = pick_stage_auto<ST>(P.mx, P.my, P.nky, P.nkx, nl, force_occ, force_thr)
     GK_BY_STORAGE(c, GK_CALL);
 #undef GK_CALL
     c->stage_fn = pick.fn;
@@ -304,7 +323,7 @@ int gk_create(const gk_grid *g, const gk_species *sp, const gk_salpha *geo, cons
           }
         }
       }
-      if (pick.occ == 2 && !in_smem && attempt == 0) { want_occ = 1; continue; }
+      if (pick.occ == 2 && !in_smem && attempt == 0) { force_occ = 1; continue; }
       if (!rc_best) return fail(c, GK_EUNSUPPORTED, "padded grid does not fit the shared-memory strategy");
       P.rc = rc_best;
       P.gchi_in_smem = in_smem;

@@ -186,15 +186,27 @@ gk_stage_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkStage
   float2 *chis = A.chis + (long long)blockIdx.x * 3 * slab;  // chi0, D_s chi (v>0), D_s chi (v<0)
   __syncthreads();
 
+  constexpr int KC = (NKX_ - 1) / 2;  // compile-time K of the specialised kernels
   // real-space gradients of the spectral slab `g` (callable: slab index -> value), chunk by chunk
   auto to_real = [&](auto g, auto sink) {
-    gkfft::inv_nat2perm_load<MX_>(mx, SA, 2 * nky, 1, ldx, twx, tid, nthr, [&](int c, int n) {
+    gkfft::inv_nat2perm_load<MX_>(mx, SA, 2 * nky, 1, ldx, twx, tid, nthr,
+                                  [&](int c, int nbase, auto offc, auto spanc) {
+      constexpr int off = decltype(offc)::value, hi = off + decltype(spanc)::value - 1;
+      const int n = nbase + off;
+      int p;
+      if constexpr (SPEC && hi <= KC) {
+        p = n;                                   // always a retained kx >= 0
+      } else if constexpr (SPEC && (off > KC && hi < MX_ - KC)) {
+        return make_float2(0.f, 0.f);            // always zero padding: nothing is loaded
+      } else if constexpr (SPEC && off >= MX_ - KC) {
+        p = n - mx;                              // always a retained kx < 0
+      } else {
+        if (n <= K) p = n;
+        else if (n >= mx - K) p = n - mx;
+        else return make_float2(0.f, 0.f);
+      }
       const bool isx = c < nky;
       const int m = isx ? c : c - nky;
-      int p;
-      if (n <= K) p = n;
-      else if (n >= mx - K) p = n - mx;
-      else return make_float2(0.f, 0.f);
       float2 v = g((p + K) * nky + m);
       if (isx) {
         const float kxv = (float)p * P.dkx;
@@ -204,21 +216,35 @@ gk_stage_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkStage
     });
     __syncthreads();
     for (int r0 = 0; r0 < mx; r0 += rc) {
-      gkfft::inv_nat2perm_load<MY_>(my, SW, rc, ldy, 1, twy, tid, nthr, [&](int r, int y) {
+      gkfft::inv_nat2perm_load<MY_>(my, SW, rc, ldy, 1, twy, tid, nthr,
+                                    [&](int r, int nbase, auto offc, auto spanc) {
+        constexpr int off = decltype(offc)::value, span = decltype(spanc)::value, hi = off + span - 1;
+        const int y = nbase + off;
         const float2 *row = SA + (r0 + r) * ldx;
-        if (y == 0) return make_float2(row[0].x, 0.f);
-        if (y < nky) {                       // X + i (i ky Y0)
-          const float kyv = (float)y * P.ky0;
-          const float2 ax = row[y], g0 = row[nky + y];
+        auto lower = [&](int m) {                // X + i (i ky Y0)
+          const float kyv = (float)m * P.ky0;
+          const float2 ax = row[m], g0 = row[nky + m];
           return make_float2(ax.x - kyv * g0.x, ax.y - kyv * g0.y);
-        }
-        if (y > my - nky) {                  // conj(X) + i conj(i ky Y0)
-          const int m = my - y;
+        };
+        auto upper = [&](int m) {                // conj(X) + i conj(i ky Y0)
           const float kyv = (float)m * P.ky0;
           const float2 ax = row[m], g0 = row[nky + m];
           return make_float2(ax.x + kyv * g0.x, -(ax.y + kyv * g0.y));
+        };
+        if constexpr (SPEC && off == 0 && span == 1) {
+          return make_float2(row[0].x, 0.f);     // ky = 0: real part only (R15)
+        } else if constexpr (SPEC && off > 0 && hi < NKY_) {
+          return lower(y);
+        } else if constexpr (SPEC && off >= NKY_ && hi <= MY_ - NKY_) {
+          return make_float2(0.f, 0.f);
+        } else if constexpr (SPEC && off > MY_ - NKY_) {
+          return upper(my - y);
+        } else {
+          if (y == 0) return make_float2(row[0].x, 0.f);
+          if (y < nky) return lower(y);
+          if (y > my - nky) return upper(my - y);
+          return make_float2(0.f, 0.f);
         }
-        return make_float2(0.f, 0.f);
       });
       __syncthreads();
       sink(r0);
@@ -280,15 +306,36 @@ gk_stage_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkStage
       if (NL) {
         to_real([&](int e) { return Cv<ST>::ldg(A.y, C.base + e); },
                 [&](int r0) {
-                  // bracket d_y chi d_x f - d_x chi d_y f; rows (p, p+rc/2) packed as (re, im)
-                  for (int q = tid; q < half * my; q += nthr) {
-                    const int p = q / my, y = q - p * my;
-                    const float2 g0 = SG[(r0 + p) * ldy + y], g1 = SG[(r0 + p + half) * ldy + y];
-                    const float2 f0 = SW[p * ldy + y], f1 = SW[(p + half) * ldy + y];
-                    SW[p * ldy + y] = make_float2(g0.y * f0.x - g0.x * f0.y, g1.y * f1.x - g1.x * f1.y);
+                  // bracket d_y chi d_x f - d_x chi d_y f, rows (p, p+rc/2) packed as (re, im), evaluated
+                  // inside the first pass of the forward y-transform; only the retained ky are stored
+                  auto keep = [&](int p, int nbase, auto offc, auto spanc, float2 v) {
+                    constexpr int off = decltype(offc)::value, hi = off + decltype(spanc)::value - 1;
+                    const int m = nbase + off;
+                    if constexpr (SPEC && off >= NKY_ && hi <= MY_ - NKY_) {
+                    } else if constexpr (SPEC && (hi < NKY_ || off > MY_ - NKY_)) {
+                      SW[p * ldy + m] = v;
+                    } else {
+                      if (m < nky || m > my - nky) SW[p * ldy + m] = v;
+                    }
+                  };
+                  if (P.gchi_in_smem) {
+                    gkfft::fwd_perm2nat_fused<MY_>(my, SW, half, ldy, 1, twy, tid, nthr,
+                        [&](int p, int q) {
+                          const float2 g0 = SG[(r0 + p) * ldy + q], g1 = SG[(r0 + p + half) * ldy + q];
+                          const float2 f0 = SW[p * ldy + q], f1 = SW[(p + half) * ldy + q];
+                          return make_float2(g0.y * f0.x - g0.x * f0.y, g1.y * f1.x - g1.x * f1.y);
+                        }, keep);
+                  } else {  // grad(chi) in global scratch: coalesced product pass (lane = y) first
+                    for (int q = tid; q < half * my; q += nthr) {
+                      const int p = q / my, y = q - p * my;
+                      const float2 g0 = SG[(r0 + p) * ldy + y], g1 = SG[(r0 + p + half) * ldy + y];
+                      const float2 f0 = SW[p * ldy + y], f1 = SW[(p + half) * ldy + y];
+                      SW[p * ldy + y] = make_float2(g0.y * f0.x - g0.x * f0.y, g1.y * f1.x - g1.x * f1.y);
+                    }
+                    __syncthreads();
+                    gkfft::fwd_perm2nat_fused<MY_>(my, SW, half, ldy, 1, twy, tid, nthr,
+                        [&](int p, int q) { return SW[p * ldy + q]; }, keep);
                   }
-                  __syncthreads();
-                  gkfft::fwd_perm2nat<MY_>(my, SW, half, ldy, 1, twy, tid, nthr);
                   __syncthreads();
                   // unpack the two real rows, keep only the retained ky: overwrite A's X columns
                   for (int q = tid; q < half * nky; q += nthr) {
@@ -300,7 +347,19 @@ gk_stage_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkStage
                     SA[(r0 + p + half) * ldx + m] = make_float2(z.y - zc.y, zc.x - z.x);
                   }
                 });
-        gkfft::fwd_perm2nat<MX_>(mx, SA, nky, 1, ldx, twx, tid, nthr);
+        // forward x-transform of the nky columns; only |p| <= K is stored
+        gkfft::fwd_perm2nat_fused<MX_>(mx, SA, nky, 1, ldx, twx, tid, nthr,
+            [&](int c, int q) { return SA[q * ldx + c]; },
+            [&](int c, int nbase, auto offc, auto spanc, float2 v) {
+              constexpr int off = decltype(offc)::value, hi = off + decltype(spanc)::value - 1;
+              const int n = nbase + off;
+              if constexpr (SPEC && (off > KC && hi < MX_ - KC)) {
+              } else if constexpr (SPEC && (hi <= KC || off >= MX_ - KC)) {
+                SA[n * ldx + c] = v;
+              } else {
+                if (n <= K || n >= mx - K) SA[n * ldx + c] = v;
+              }
+            });
         __syncthreads();
       }
       // ---- epilogue: one coalesced pass over the slab ----
