@@ -12,12 +12,21 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libgk.so")
-SOURCES = ["gk_lib.cu"]
-DEPS = ["gk_lib.cu", "gk_kernels.cuh", "gk_fft.cuh", "gk_tables.h", "gk_dev.h"]
+OBJDIR = os.path.join(HERE, "build")
+# (source, extra defines, object name): the stage kernel is instantiated once per storage type in
+# its own translation unit so that the units compile in parallel
+UNITS = [
+    ("gk_lib.cu", [], "gk_lib.o"),
+    ("gk_stage_inst.cu", ["-DGK_ST_ID=0"], "gk_stage_c64.o"),
+    ("gk_stage_inst.cu", ["-DGK_ST_ID=1"], "gk_stage_f16.o"),
+    ("gk_stage_inst.cu", ["-DGK_ST_ID=2"], "gk_stage_bf16.o"),
+]
+DEPS = ["gk_lib.cu", "gk_stage_inst.cu", "gk_kernels.cuh", "gk_common.cuh", "gk_stage.cuh", "gk_fft.cuh", "gk_tables.h",
+        "gk_dev.h", "gk_pick.h"]
 
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
-    "--shared", "-Xcompiler", "-fPIC", "-Xptxas", "-v",
+    "-Xcompiler", "-fPIC", "-Xptxas", "-v",
 ]
 
 
@@ -40,14 +49,34 @@ def build(force: bool = False, verbose: bool = False) -> str:
     """Compile if the library is missing or older than its sources; returns the library path."""
     if not force and not is_stale():
         return LIB
+    from concurrent.futures import ThreadPoolExecutor
+    os.makedirs(OBJDIR, exist_ok=True)
+    fast = bool(os.environ.get("GK_FAST_BUILD"))           # developer builds only: complex64 storage
+    units = UNITS[:2] if fast else UNITS
+    extra = ["-DGK_ONLY_C64"] if fast else []
+
+    def compile_unit(u):
+        src, defs, obj = u
+        cmd = [_nvcc(), *NVCC_FLAGS, *extra, *defs, "-c", os.path.join(CSRC, src), "-o", os.path.join(OBJDIR, obj)]
+        res = subprocess.run(cmd, capture_output=True, text=True)
+        return cmd, res
+
+    with ThreadPoolExecutor(len(units)) as ex:
+        results = list(ex.map(compile_unit, units))
+    log = ""
+    for cmd, res in results:
+        log += " ".join(cmd) + "\n" + res.stdout + res.stderr
     tmp = LIB + f".{os.getpid()}.tmp"
-    extra = ["-DGK_ONLY_C64"] if os.environ.get("GK_FAST_BUILD") else []   # developer builds only
-    cmd = [_nvcc(), *NVCC_FLAGS, *extra, *[os.path.join(CSRC, s) for s in SOURCES], "-o", tmp]
-    res = subprocess.run(cmd, capture_output=True, text=True)
-    log = res.stdout + res.stderr
+    ok = all(res.returncode == 0 for _, res in results)
+    if ok:
+        cmd = [_nvcc(), "--shared", "-gencode", "arch=compute_100a,code=sm_100a",
+               *[os.path.join(OBJDIR, u[2]) for u in units], "-o", tmp]
+        res = subprocess.run(cmd, capture_output=True, text=True)
+        log += " ".join(cmd) + "\n" + res.stdout + res.stderr
+        ok = res.returncode == 0
     with open(os.path.join(HERE, "build.log"), "w") as fh:
-        fh.write(" ".join(cmd) + "\n" + log)
-    if res.returncode != 0:
+        fh.write(log)
+    if not ok:
         sys.stderr.write(log)
         raise RuntimeError("nvcc failed building libgk.so")
     os.replace(tmp, LIB)

@@ -4,6 +4,7 @@
 #include <stdint.h>
 
 #define GK_MAX_SPECIES 4
+#define GK_SLAB_MAX 8192  // largest nkx*nky a CTA handles (moment accumulators live in registers)
 
 // Per-species scalars, float copies of the host doubles.
 struct GkSpeciesDev {

@@ -39,10 +39,19 @@ __host__ __device__ constexpr double cx_sin(double x) {
   return s;
 }
 
-__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
-__device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
-__device__ __forceinline__ float2 cmul(float2 a, float2 b) {
-  return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+// Complex arithmetic on the packed fp32x2 pipe of sm_100a (FADD2 / FMUL2 / FFMA2 take a complex
+// number per instruction; the half-swap and per-half negation that multiplication by +-i needs are
+// operand modifiers, and a real factor is a broadcast operand, so they cost nothing).
+__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return __fadd2_rn(a, b); }
+__device__ __forceinline__ float2 csub(float2 a, float2 b) { return __fadd2_rn(a, make_float2(-b.x, -b.y)); }
+// a + s*b, s real
+__device__ __forceinline__ float2 caxpy(float s, float2 b, float2 a) { return __ffma2_rn(b, make_float2(s, s), a); }
+__device__ __forceinline__ float2 cscale(float s, float2 a) { return __fmul2_rn(a, make_float2(s, s)); }
+__device__ __forceinline__ float2 cmul(float2 a, float2 b) {   // a*b = a b.x + (i a) b.y
+  return __ffma2_rn(make_float2(-a.y, a.x), make_float2(b.y, b.y), __fmul2_rn(a, make_float2(b.x, b.x)));
+}
+__device__ __forceinline__ float2 cmulc(float2 a, float2 b) {  // a*conj(b)
+  return __ffma2_rn(make_float2(a.y, -a.x), make_float2(b.y, b.y), __fmul2_rn(a, make_float2(b.x, b.x)));
 }
 // multiply by S*i
 template <int S> __device__ __forceinline__ float2 muli(float2 a) {
@@ -60,7 +69,7 @@ template <int N, int K, int S> __device__ __forceinline__ float2 mulw(float2 a) 
     constexpr double ang = 2.0 * kPi * (k > N / 2 ? k - N : k) / N;
     constexpr float c = (float)cx_cos(ang);
     constexpr float s = (float)(S * cx_sin(ang));
-    return make_float2(a.x * c - a.y * s, a.x * s + a.y * c);
+    return __ffma2_rn(make_float2(-a.y, a.x), make_float2(s, s), __fmul2_rn(a, make_float2(c, c)));
   }
 }
 
@@ -72,13 +81,12 @@ template <int R, int S> __device__ __forceinline__ void dft(float2 (&v)[R]) {
     v[0] = cadd(a, b);
     v[1] = csub(a, b);
   } else if constexpr (R == 3) {
-    float2 t1 = cadd(v[1], v[2]);
-    float2 t2 = make_float2(v[0].x - 0.5f * t1.x, v[0].y - 0.5f * t1.y);
-    float2 d = csub(v[1], v[2]);
-    float2 t3 = muli<S>(make_float2(0.86602540378443864676f * d.x, 0.86602540378443864676f * d.y));
+    const float2 t1 = cadd(v[1], v[2]);
+    const float2 t2 = caxpy(-0.5f, t1, v[0]);
+    const float2 d = muli<S>(csub(v[1], v[2]));
     v[0] = cadd(v[0], t1);
-    v[1] = cadd(t2, t3);
-    v[2] = csub(t2, t3);
+    v[1] = caxpy(0.86602540378443864676f, d, t2);
+    v[2] = caxpy(-0.86602540378443864676f, d, t2);
   } else if constexpr (R == 4) {
     float2 s02 = cadd(v[0], v[2]), d02 = csub(v[0], v[2]);
     float2 s13 = cadd(v[1], v[3]), d13 = muli<S>(csub(v[1], v[3]));
@@ -156,9 +164,8 @@ __device__ __forceinline__ void nat2perm_load(float2 *base, int nb, int bstride,
       dft<R2, S>(u);
 #pragma unroll
       for (int k2 = 1; k2 < R2; ++k2) {
-        float2 t = tw[n1 * k2];
-        if (S < 0) t.y = -t.y;
-        u[k2] = cmul(u[k2], t);
+        const float2 t = tw[n1 * k2];
+        u[k2] = S > 0 ? cmul(u[k2], t) : cmulc(u[k2], t);
       }
 #pragma unroll
       for (int k2 = 0; k2 < R2; ++k2) p[k2 * R1 * estride] = u[k2];
@@ -208,9 +215,8 @@ __device__ __forceinline__ void perm2nat_fused(float2 *base, int nb, int bstride
       dft<R1, S>(u);
 #pragma unroll
       for (int n1 = 1; n1 < R1; ++n1) {
-        float2 t = tw[n1 * k2];
-        if (S < 0) t.y = -t.y;
-        u[n1] = cmul(u[n1], t);
+        const float2 t = tw[n1 * k2];
+        u[n1] = S > 0 ? cmul(u[n1], t) : cmulc(u[n1], t);
       }
 #pragma unroll
       for (int n1 = 0; n1 < R1; ++n1) p[n1 * estride] = u[n1];

@@ -7,46 +7,9 @@
 //                      update and the moment planes of the next stage, one pass over f
 //   gk_flux_kernel     diagnostics
 #pragma once
-#include <cuda_bf16.h>
-#include <cuda_fp16.h>
-
-#include "gk_dev.h"
-#include "gk_fft.cuh"
-
-#define GK_T_I 1
-#define GK_T_II 2
-#define GK_T_IV 4
-#define GK_T_V 8
-#define GK_T_VII 16
-#define GK_T_VIII 32
-#define GK_T_DISS_S 64
-#define GK_T_DISS_V 128
-#define GK_T_HYP 256
-#define GK_T_III 512
+#include "gk_common.cuh"
 
 namespace gk {
-
-using gkfft::cadd;
-using gkfft::cmul;
-using gkfft::csub;
-
-// ---- storage types: complex64 / complex fp16 / complex bf16, arithmetic always fp32 (R19) ----
-template <class ST> struct Cv;
-template <> struct Cv<float2> {
-  static __device__ __forceinline__ float2 ld(const void *p, long long i) { return ((const float2 *)p)[i]; }
-  static __device__ __forceinline__ float2 ldg(const void *p, long long i) { return __ldg((const float2 *)p + i); }
-  static __device__ __forceinline__ void st(void *p, long long i, float2 v) { ((float2 *)p)[i] = v; }
-};
-template <> struct Cv<__half2> {
-  static __device__ __forceinline__ float2 ld(const void *p, long long i) { return __half22float2(((const __half2 *)p)[i]); }
-  static __device__ __forceinline__ float2 ldg(const void *p, long long i) { return __half22float2(__ldg((const __half2 *)p + i)); }
-  static __device__ __forceinline__ void st(void *p, long long i, float2 v) { ((__half2 *)p)[i] = __float22half2_rn(v); }
-};
-template <> struct Cv<__nv_bfloat162> {
-  static __device__ __forceinline__ float2 ld(const void *p, long long i) { return __bfloat1622float2(((const __nv_bfloat162 *)p)[i]); }
-  static __device__ __forceinline__ float2 ldg(const void *p, long long i) { return __bfloat1622float2(((const __nv_bfloat162 *)p)[i]); }
-  static __device__ __forceinline__ void st(void *p, long long i, float2 v) { ((__nv_bfloat162 *)p)[i] = __float22bfloat162_rn(v); }
-};
 
 // =================================================================================================
 // a1. Velocity-space moment.  One thread per (work item, slab element); a work
@@ -158,4 +121,3 @@ __global__ void __launch_bounds__(256) gk_flux_kernel(const __grid_constant__ Gk
 
 }  // namespace gk
 
-#include "gk_stage.cuh"

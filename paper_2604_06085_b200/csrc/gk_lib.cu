@@ -8,6 +8,7 @@
 
 #include "../../include/gk.h"
 #include "gk_kernels.cuh"
+#include "gk_pick.h"
 #include "gk_tables.h"
 
 namespace {
@@ -97,37 +98,6 @@ template <class ST> void launch_moment(gk_ctx *c, const void *f, float2 *mom) {
   const long long nwork = (long long)P.nsp * P.nmu * P.nchunk * P.ns;
   gk::gk_moment_kernel<ST><<<(unsigned)(nwork * nblk_slab), 256, 0, c->stream>>>(P, f, mom);
   ++c->launches;
-}
-
-// Stage-kernel instantiations: the four BASELINE shapes get compile-time sizes (index arithmetic and
-// FFT radices fold to constants); everything else runs the generic kernel.  occ = 2 variants keep
-// grad(chi) in global scratch so that two 256-thread CTAs share an SM.
-struct StagePick { const void *fn; int threads; int occ; };
-template <class ST> StagePick pick_stage(int mx, int my, int nky, int nkx, bool nl, int want_occ, int want_thr) {
-  if (!nl) return {(const void *)gk::gk_stage_kernel<ST, 0, 0, 0, 0, false, 512, 1>, 512, 1};
-#define GK_SPEC(MX, MY, NKY, NKX, NT, OCC)                                                       \
-  if (mx == MX && my == MY && nky == NKY && nkx == NKX && want_occ == OCC && want_thr == NT)     \
-    return {(const void *)gk::gk_stage_kernel<ST, MX, MY, NKY, NKX, true, NT, OCC>, NT, OCC}
-  GK_SPEC(16, 12, 4, 9, 512, 1);
-  GK_SPEC(128, 48, 16, 85, 1024, 1);
-  GK_SPEC(128, 48, 16, 85, 512, 2);
-  GK_SPEC(128, 96, 32, 85, 1024, 1);
-  GK_SPEC(128, 96, 32, 85, 512, 1);
-  GK_SPEC(192, 192, 64, 127, 1024, 1);
-  GK_SPEC(192, 192, 64, 127, 512, 1);
-#undef GK_SPEC
-  return {nullptr, 0, 0};
-}
-// preference order of (threads, occ) variants; the first one that exists and fits is used
-template <class ST> StagePick pick_stage_auto(int mx, int my, int nky, int nkx, bool nl, int force_occ, int force_thr) {
-  static const int pref[][2] = {{1024, 1}, {512, 2}, {512, 1}};
-  for (auto &pr : pref) {
-    if (force_thr && pr[0] != force_thr) continue;
-    if (force_occ && pr[1] != force_occ) continue;
-    StagePick p = pick_stage<ST>(mx, my, nky, nkx, nl, pr[1], pr[0]);
-    if (p.fn) return p;
-  }
-  return {(const void *)gk::gk_stage_kernel<ST, 0, 0, 0, 0, true, 512, 1>, 512, 1};
 }
 
 void launch_stage(gk_ctx *c, const GkStageArgs &A) {
@@ -285,21 +255,27 @@ int gk_create(const gk_grid *g, const gk_species *sp, const gk_salpha *geo, cons
   long long nwork = 0;
   for (int attempt = 0; attempt < 2; ++attempt) {
     StagePick pick;
-#define GK_CALL(ST) pick = pick_stage_auto<ST>(P.mx, P.my, P.nky, P.nkx, nl, force_occ, force_thr)
-    GK_BY_STORAGE(c, GK_CALL);
-#undef GK_CALL
+    pick = gk_pick_stage(o->storage, P.mx, P.my, P.nky, P.nkx, nl, force_occ, force_thr);
+    if (!pick.fn) return fail(c, GK_EUNSUPPORTED, "this build has no stage kernel for the requested storage");
     c->stage_fn = pick.fn;
     c->stage_threads = pick.threads;
     c->stage_occ = pick.occ;
     const int resident = c->num_sms * pick.occ;  // persistent CTAs
 
-    // work decomposition: >= 6 work items per resident CTA, vpar chunks >= 4 long
+    // work decomposition: items (a, l, vpar chunk, i) are dealt round-robin to the persistent CTAs.
+    // Cost of a split = rounds x (slabs per item + the chi build of the item, in slab units);
+    // chunks stay >= 4 long so that chi is amortised.
     {
       const long long ali = (long long)T.nsp * T.nmu * T.ns;
-      long long nchunk = (6LL * resident + ali - 1) / ali;
-      nchunk = std::max<long long>(1, std::min<long long>(nchunk, T.nv / 4));
-      P.jchunk = (int)((T.nv + nchunk - 1) / nchunk);
-      P.nchunk = (T.nv + P.jchunk - 1) / P.jchunk;
+      const double chi_cost = nl ? 0.7 : 0.3;
+      double best = 1e300;
+      for (int nch = 1; nch <= std::max(1, T.nv / 4); ++nch) {
+        const int jc = (T.nv + nch - 1) / nch;
+        const int nce = (T.nv + jc - 1) / jc;
+        const long long rounds = (ali * nce + resident - 1) / resident;
+        const double cost = (double)rounds * (jc + chi_cost);
+        if (cost < best - 1e-9) { best = cost; P.jchunk = jc; P.nchunk = nce; }
+      }
       P.nparts = T.nsp * T.nmu * P.nchunk;
     }
     nwork = (long long)T.nsp * T.nmu * T.ns * P.nchunk;
@@ -333,7 +309,7 @@ int gk_create(const gk_grid *g, const gk_species *sp, const gk_salpha *geo, cons
       P.rc = 2;
       P.gchi_in_smem = 1;
       c->stage_smem = (size_t)P.slab * 8;
-      c->stage_grid = (int)std::min<long long>(nwork, 2LL * c->num_sms);
+      c->stage_grid = (int)std::min<long long>(nwork, resident);
     }
     break;
   }

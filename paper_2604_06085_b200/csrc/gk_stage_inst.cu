@@ -1,0 +1,66 @@
+// gk_stage_inst.cu -- instantiations of gk_stage_kernel for one storage type (GK_ST_ID = 0 complex64,
+// 1 complex fp16, 2 complex bf16).  Product path.
+#include "gk_common.cuh"
+#include "gk_stage.cuh"
+#include "gk_pick.h"
+
+#ifndef GK_ST_ID
+#define GK_ST_ID 0
+#endif
+#if GK_ST_ID == 0
+#define GK_ST float2
+#define GK_PICK_NAME gk_pick_stage_c64
+#elif GK_ST_ID == 1
+#define GK_ST __half2
+#define GK_PICK_NAME gk_pick_stage_f16
+#else
+#define GK_ST __nv_bfloat162
+#define GK_PICK_NAME gk_pick_stage_bf16
+#endif
+
+namespace {
+
+// Stage-kernel instantiations: the four BASELINE shapes get compile-time sizes (index arithmetic and
+// FFT radices fold to constants); everything else runs the generic kernel.  occ = 2 variants keep
+// grad(chi) in global scratch so that two 256-thread CTAs share an SM.
+template <class ST> StagePick pick_stage(int mx, int my, int nky, int nkx, bool nl, int want_occ, int want_thr) {
+#define GK_SPEC(MX, MY, NKY, NKX, NT, OCC)                                                       \
+  if (nl && mx == MX && my == MY && nky == NKY && nkx == NKX && want_occ == OCC && want_thr == NT) \
+    return {(const void *)gk::gk_stage_kernel<ST, MX, MY, NKY, NKX, true, NT, OCC>, NT, OCC}
+  GK_SPEC(16, 12, 4, 9, 512, 1);
+  GK_SPEC(128, 48, 16, 85, 1024, 1);
+  GK_SPEC(128, 48, 16, 85, 512, 2);
+  GK_SPEC(128, 96, 32, 85, 1024, 1);
+  GK_SPEC(128, 96, 32, 85, 512, 1);
+  GK_SPEC(192, 192, 64, 127, 1024, 1);
+  GK_SPEC(192, 192, 64, 127, 512, 1);
+#undef GK_SPEC
+  // term III switched off: a streaming stencil kernel
+#define GK_SPEC_LIN(NKY, NKX)                                                                    \
+  if (!nl && nky == NKY && nkx == NKX && want_occ == 1 && want_thr == 1024)                      \
+    return {(const void *)gk::gk_stage_kernel<ST, 0, 0, NKY, NKX, false, 1024, 1>, 1024, 1}
+  GK_SPEC_LIN(16, 85);
+  GK_SPEC_LIN(32, 85);
+  GK_SPEC_LIN(64, 127);
+#undef GK_SPEC_LIN
+  return {nullptr, 0, 0};
+}
+// preference order of (threads, occ) variants; the first one that exists and fits is used
+template <class ST> StagePick pick_stage_auto(int mx, int my, int nky, int nkx, bool nl, int force_occ, int force_thr) {
+  static const int pref[][2] = {{1024, 1}, {512, 2}, {512, 1}};
+  for (auto &pr : pref) {
+    if (force_thr && pr[0] != force_thr) continue;
+    if (force_occ && pr[1] != force_occ) continue;
+    StagePick p = pick_stage<ST>(mx, my, nky, nkx, nl, pr[1], pr[0]);
+    if (p.fn) return p;
+  }
+  if (!nl) return {(const void *)gk::gk_stage_kernel<ST, 0, 0, 0, 0, false, 512, 1>, 512, 1};
+  return {(const void *)gk::gk_stage_kernel<ST, 0, 0, 0, 0, true, 512, 1>, 512, 1};
+}
+
+
+}  // namespace
+
+StagePick GK_PICK_NAME(int mx, int my, int nky, int nkx, bool nl, int force_occ, int force_thr) {
+  return pick_stage_auto<GK_ST>(mx, my, nky, nkx, nl, force_occ, force_thr);
+}
