@@ -23,6 +23,7 @@ struct GkDev {
   int adiabatic, mask, storage;
   int jchunk, nchunk;  // vpar chunking of the stage kernel's work items
   int nparts;          // number of moment partial planes = nsp*nmu*nchunk
+  int prefetch;        // 1: L2 prefetch of the single-use epilogue operands before the FFT phase
   int gchi_in_smem;    // 1: real-space grad(chi) lives in shared memory, 0: per-CTA global scratch
   float ds_inv, dv_inv;
   float dkx, ky0;      // kx_p = p*dkx, ky_m = m*ky0
@@ -60,6 +61,8 @@ struct GkStageArgs {
   float2 *mom;       // moment partial planes of `out` (nullptr: skip)
   float2 *gchi;      // per-CTA scratch for real-space grad(chi) when !gchi_in_smem
   float2 *chis;      // per-CTA scratch, 3*slab: chi = J0 phi, D_s chi for v>0, D_s chi for v<0
+                     // (warp-specialised kernel: a ring of 3 such triples)
+  float2 *nlbuf;     // warp-specialised kernel: per-CTA ring of 2 bracket slabs
   float c, b;        // y_next = base + c*k ; acc (+)= b*k     (dt folded in)
   int mode;          // 0: out = k; 1: acc = y + b k, out = y + c k; 2: acc += b k, out = fn + c k;
                      // 3: out = acc + b k

@@ -148,9 +148,18 @@ GK_FAC(64, 8, 8); GK_FAC(96, 8, 12); GK_FAC(128, 8, 16); GK_FAC(192, 12, 16); GK
 // nat2perm_load:  natural-order input of batch b from LOAD(b, nbase, IC<OFF>, IC<SPAN>) (global
 //   memory, or another shared array combined on the fly): the first radix pass doubles as the
 //   load / zero-pad / pre-multiply pass.  Output digit-permuted in `base`.
-template <int N, int S, class LOAD>
+struct CtaSync { __device__ __forceinline__ void operator()() const { __syncthreads(); } };
+// barrier among the NTHR threads (a multiple of 32) that name the same id
+template <int ID, int NTHR> struct NamedSync {
+  __device__ __forceinline__ void operator()() const {
+    asm volatile("bar.sync %0, %1;" ::"n"(ID), "n"(NTHR) : "memory");
+  }
+};
+
+template <int N, int S, class LOAD, class SYNC = CtaSync>
 __device__ __forceinline__ void nat2perm_load(float2 *base, int nb, int bstride, int estride,
-                                              const float2 *tw, int tid, int nthr, LOAD load) {
+                                              const float2 *tw, int tid, int nthr, LOAD load,
+                                              SYNC sync = SYNC{}) {
   constexpr int R1 = Fac<N>::R1, R2 = Fac<N>::R2;
   if constexpr (R2 > 1) {
     for (int w = tid; w < nb * R1; w += nthr) {
@@ -170,7 +179,7 @@ __device__ __forceinline__ void nat2perm_load(float2 *base, int nb, int bstride,
 #pragma unroll
       for (int k2 = 0; k2 < R2; ++k2) p[k2 * R1 * estride] = u[k2];
     }
-    __syncthreads();
+    sync();
     for (int w = tid; w < nb * R2; w += nthr) {
       const int b = w % nb, k2 = w / nb;
       float2 *p = base + b * bstride + k2 * R1 * estride;
@@ -200,10 +209,10 @@ __device__ __forceinline__ void nat2perm_load(float2 *base, int nb, int bstride,
 //   several shared arrays: the pointwise bracket is evaluated here); natural-order output handed
 //   to STORE(b, nbase, IC<OFF>, IC<SPAN>, value).  `base` is the exchange buffer between the
 //   two radix passes; LOADP may read it at the positions its own work item overwrites.
-template <int N, int S, class LOADP, class STORE>
+template <int N, int S, class LOADP, class STORE, class SYNC = CtaSync>
 __device__ __forceinline__ void perm2nat_fused(float2 *base, int nb, int bstride, int estride,
                                                const float2 *tw, int tid, int nthr, LOADP loadp,
-                                               STORE store) {
+                                               STORE store, SYNC sync = SYNC{}) {
   constexpr int R1 = Fac<N>::R1, R2 = Fac<N>::R2;
   if constexpr (R2 > 1) {
     for (int w = tid; w < nb * R2; w += nthr) {
@@ -221,7 +230,7 @@ __device__ __forceinline__ void perm2nat_fused(float2 *base, int nb, int bstride
 #pragma unroll
       for (int n1 = 0; n1 < R1; ++n1) p[n1 * estride] = u[n1];
     }
-    __syncthreads();
+    sync();
     for (int w = tid; w < nb * R1; w += nthr) {
       const int b = w % nb, n1 = w / nb;
       const float2 *p = base + b * bstride + n1 * estride;
@@ -259,25 +268,26 @@ __device__ __forceinline__ void perm2nat_fused(float2 *base, int nb, int bstride
   }
 
 // Size dispatch: NC > 0 is a compile-time length (specialised kernels), NC == 0 switches on n.
-template <int NC, class LOAD>
+template <int NC, class LOAD, class SYNC = CtaSync>
 __device__ __forceinline__ void inv_nat2perm_load(int n, float2 *base, int nb, int bstride, int estride,
-                                                  const float2 *tw, int tid, int nthr, LOAD load) {
+                                                  const float2 *tw, int tid, int nthr, LOAD load,
+                                                  SYNC sync = SYNC{}) {
   if constexpr (NC > 0) {
-    nat2perm_load<NC, +1>(base, nb, bstride, estride, tw, tid, nthr, load);
+    nat2perm_load<NC, +1>(base, nb, bstride, estride, tw, tid, nthr, load, sync);
   } else {
-#define GK_CALL(N_) nat2perm_load<N_, +1>(base, nb, bstride, estride, tw, tid, nthr, load)
+#define GK_CALL(N_) nat2perm_load<N_, +1>(base, nb, bstride, estride, tw, tid, nthr, load, sync)
     GK_FFT_SWITCH(n, GK_CALL)
 #undef GK_CALL
   }
 }
-template <int NC, class LOADP, class STORE>
+template <int NC, class LOADP, class STORE, class SYNC = CtaSync>
 __device__ __forceinline__ void fwd_perm2nat_fused(int n, float2 *base, int nb, int bstride, int estride,
                                                    const float2 *tw, int tid, int nthr, LOADP loadp,
-                                                   STORE store) {
+                                                   STORE store, SYNC sync = SYNC{}) {
   if constexpr (NC > 0) {
-    perm2nat_fused<NC, -1>(base, nb, bstride, estride, tw, tid, nthr, loadp, store);
+    perm2nat_fused<NC, -1>(base, nb, bstride, estride, tw, tid, nthr, loadp, store, sync);
   } else {
-#define GK_CALL(N_) perm2nat_fused<N_, -1>(base, nb, bstride, estride, tw, tid, nthr, loadp, store)
+#define GK_CALL(N_) perm2nat_fused<N_, -1>(base, nb, bstride, estride, tw, tid, nthr, loadp, store, sync)
     GK_FFT_SWITCH(n, GK_CALL)
 #undef GK_CALL
   }

@@ -37,13 +37,13 @@ struct gk_ctx {
   bool poisoned = false;
   int num_sms = 0;
   int stage_grid = 0;
-  int stage_threads = 512, stage_occ = 1;
+  int stage_threads = 512, stage_occ = 1, stage_ws = 0;
   size_t stage_smem = 0;
   size_t elem_bytes = 8;
   // workspace
   void *ws = nullptr;
   size_t ws_bytes = 0;
-  size_t off_mom = 0, off_phi = 0, off_gchi = 0, off_chis = 0, off_ya = 0, off_yb = 0, off_acc = 0;
+  size_t off_mom = 0, off_phi = 0, off_gchi = 0, off_chis = 0, off_nl = 0, off_ya = 0, off_yb = 0, off_acc = 0;
   const void *stage_fn = nullptr;  // the gk_stage_kernel instantiation chosen at create time
   size_t need_rhs = 0, need_full = 0;
   bool mom_valid_for_f = false;  // inside gk_rk4_steps only
@@ -243,6 +243,8 @@ int gk_create(const gk_grid *g, const gk_species *sp, const gk_salpha *geo, cons
     if (P.mx % 2) return fail(c, GK_EUNSUPPORTED, "padded x size must be even (row pairs)");
   }
   P.fftnorm = (float)(1.0 / ((double)P.mx * P.my));
+  P.prefetch = 1;
+  if (const char *env = std::getenv("GK_PREFETCH")) P.prefetch = std::atoi(env);
   P.ldx = 2 * T.nky + 1;
   P.ldy = P.my | 1;
 
@@ -252,14 +254,19 @@ int gk_create(const gk_grid *g, const gk_species *sp, const gk_salpha *geo, cons
   int force_occ = 0, force_thr = 0;
   if (const char *env = std::getenv("GK_STAGE_OCC")) force_occ = std::atoi(env);
   if (const char *env = std::getenv("GK_STAGE_THREADS")) force_thr = std::atoi(env);
+  // warp-specialised kernel (FFT warps + epilogue warps): GK_WS_NTF = FFT-role threads, 0 = unified kernel
+  int ws_ntf = 512;
+  if (const char *env = std::getenv("GK_WS_NTF")) ws_ntf = std::atoi(env);
+  if (force_occ || force_thr) ws_ntf = 0;
   long long nwork = 0;
   for (int attempt = 0; attempt < 2; ++attempt) {
     StagePick pick;
-    pick = gk_pick_stage(o->storage, P.mx, P.my, P.nky, P.nkx, nl, force_occ, force_thr);
+    pick = gk_pick_stage(o->storage, P.mx, P.my, P.nky, P.nkx, nl, force_occ, force_thr, ws_ntf);
     if (!pick.fn) return fail(c, GK_EUNSUPPORTED, "this build has no stage kernel for the requested storage");
     c->stage_fn = pick.fn;
     c->stage_threads = pick.threads;
     c->stage_occ = pick.occ;
+    c->stage_ws = pick.ws;
     const int resident = c->num_sms * pick.occ;  // persistent CTAs
 
     // work decomposition: items (a, l, vpar chunk, i) are dealt round-robin to the persistent CTAs.
@@ -299,7 +306,7 @@ int gk_create(const gk_grid *g, const gk_species *sp, const gk_salpha *geo, cons
           }
         }
       }
-      if (pick.occ == 2 && !in_smem && attempt == 0) { force_occ = 1; continue; }
+      if (pick.occ == 2 && !in_smem && attempt == 0 && !std::getenv("GK_STAGE_OCC")) { force_occ = 1; continue; }
       if (!rc_best) return fail(c, GK_EUNSUPPORTED, "padded grid does not fit the shared-memory strategy");
       P.rc = rc_best;
       P.gchi_in_smem = in_smem;
@@ -345,7 +352,9 @@ int gk_create(const gk_grid *g, const gk_species *sp, const gk_salpha *geo, cons
   c->off_phi = off; off += align256((size_t)P.nphi * 8);
   c->off_gchi = off;
   if (nl && !P.gchi_in_smem) off += align256((size_t)c->stage_grid * P.mx * P.ldy * 8);
-  c->off_chis = off; off += align256((size_t)c->stage_grid * 3 * P.slab * 8);
+  c->off_chis = off; off += align256((size_t)c->stage_grid * (c->stage_ws ? 9 : 3) * P.slab * 8);
+  c->off_nl = off;
+  if (c->stage_ws) off += align256((size_t)c->stage_grid * 2 * P.slab * 8);
   c->need_rhs = off;
   c->off_ya = off; off += align256((size_t)P.ntot * c->elem_bytes);
   c->off_yb = off; off += align256((size_t)P.ntot * c->elem_bytes);
@@ -392,6 +401,7 @@ int gk_rhs(gk_ctx *c, const void *f, void *phi, void *rhs) {
   A.y = f; A.out = rhs; A.phi = (const float2 *)phi; A.mode = 0;
   A.gchi = (float2 *)((char *)c->ws + c->off_gchi);
   A.chis = (float2 *)((char *)c->ws + c->off_chis);
+  A.nlbuf = (float2 *)((char *)c->ws + c->off_nl);
   A.nwork = c->P.nsp * c->P.nmu * c->P.ns * c->P.nchunk;
   stage_launch(c, A);
   return check_launch(c, "stage kernel");
@@ -410,6 +420,7 @@ int gk_rk4_steps(gk_ctx *c, void *f, double dt, int nsteps) {
   A.phi = phi; A.mom = mom; A.acc = acc;
   A.gchi = (float2 *)(ws + c->off_gchi);
   A.chis = (float2 *)(ws + c->off_chis);
+  A.nlbuf = (float2 *)(ws + c->off_nl);
   A.nwork = c->P.nsp * c->P.nmu * c->P.ns * c->P.nchunk;
   const float h = (float)dt;
   for (int s = 0; s < nsteps; ++s) {
@@ -481,7 +492,7 @@ size_t gk_export_table(const gk_ctx *c, const char *which, double *out, size_t m
   } else if (w == "pad") {
     tmp = {(double)c->P.mx, (double)c->P.my, (double)c->P.rc, (double)c->P.gchi_in_smem,
            (double)c->P.jchunk, (double)c->P.nchunk, (double)c->stage_grid, (double)c->stage_smem,
-           (double)c->stage_threads, (double)c->stage_occ};
+           (double)c->stage_threads, (double)c->stage_occ, (double)c->stage_ws};
     src = &tmp;
   } else return 0;
   if (out) std::memcpy(out, src->data(), std::min(maxn, src->size()) * sizeof(double));

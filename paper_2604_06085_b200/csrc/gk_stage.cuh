@@ -117,6 +117,125 @@ __device__ __forceinline__ bool seam_offset(const GkDev &P, int i, int d, int ip
   return ok;
 }
 
+// Operand pointers of one slab's epilogue.
+template <class ST> struct EpiPtrs {
+  const ST *yb;                    // state slab (a,j,l,i)
+  const ST *yv0, *yv1, *yv3, *yv4; // vpar neighbours j-2, j-1, j+1, j+2 (== yb where outside the grid)
+  const ST *fnb;                   // f_n slab
+  ST *accb, *outb;                 // accumulator and output slabs
+  const float2 *chi0, *dsch;       // chi and D_s chi (for the sign of v_j) of this (a,l,i)
+};
+template <class ST>
+__device__ __forceinline__ void make_epi_ptrs(const GkStageArgs &A, const SlabCtx &C, const float2 *chis,
+                                              int slab, EpiPtrs<ST> &Q) {
+  Q.yb = (const ST *)A.y + C.base;
+  Q.yv0 = Q.yb + C.ov[0]; Q.yv1 = Q.yb + C.ov[1]; Q.yv3 = Q.yb + C.ov[2]; Q.yv4 = Q.yb + C.ov[3];
+  Q.fnb = (const ST *)A.fn + C.base;
+  Q.accb = (ST *)A.acc + C.base;
+  Q.outb = (ST *)A.out + C.base;
+  Q.chi0 = chis;
+  Q.dsch = chis + (1 + C.sg) * slab;
+}
+
+// ---- one slab element: linear terms + bracket + RK update.  The operands (own value, 4 parallel
+// and 4 vpar neighbours, f_n, accumulator, chi, D_s chi) are all requested before the arithmetic;
+// the arithmetic is one packed-fp32 FMA per operand.  INTERIOR: 2 <= i < ns-2, where the parallel
+// stencil never crosses the seam (28 of 32 planes in the BASELINE grids).  nlv: bracket value
+// (unscaled) of this element. ----
+template <class ST, int MODE, bool INTERIOR>
+__device__ __forceinline__ float2 rhs_point(const GkDev &P, const GkStageArgs &A, const ItemCtx &I,
+                                            const SlabCtx &C, const EpiPtrs<ST> &Q, int slab, int e,
+                                            int ip, int m, float pk, float fmf, float2 nlv, float scale) {
+  const float2 f0 = Cv<ST>::ldg(Q.yb, e);
+  float2 fs[5];
+  float wsd[5];
+  if constexpr (INTERIOR) {
+    fs[0] = Cv<ST>::ldg(Q.yb, e - 2 * slab);
+    fs[1] = Cv<ST>::ldg(Q.yb, e - slab);
+    fs[3] = Cv<ST>::ldg(Q.yb, e + slab);
+    fs[4] = Cv<ST>::ldg(Q.yb, e + 2 * slab);
+#pragma unroll
+    for (int d = 0; d < 5; ++d) wsd[d] = C.ws[d];
+  } else {
+    const int cls = stencil_class(P, I.i, ip, m);
+#pragma unroll
+    for (int d = 0; d < 5; ++d) {
+      const float wgt = C.cI * P.dcoef[cls][C.sg][d] + C.cDs * P.discoef[cls][d];
+      if (d == 2) { wsd[d] = wgt; continue; }
+      int off;
+      const bool ok = seam_offset(P, I.i, d - 2, ip, m, off);
+      fs[d] = Cv<ST>::ldg(Q.yb, e + off);
+      wsd[d] = ok ? wgt : 0.f;
+    }
+  }
+  const float2 fv0 = Cv<ST>::ldg(Q.yv0, e), fv1 = Cv<ST>::ldg(Q.yv1, e);
+  const float2 fv3 = Cv<ST>::ldg(Q.yv3, e), fv4 = Cv<ST>::ldg(Q.yv4, e);
+  float2 fn = f0, ac = make_float2(0.f, 0.f);
+  if constexpr (MODE == 2) fn = Cv<ST>::ldcs(Q.fnb, e);
+  if constexpr (MODE >= 2) ac = Cv<ST>::ldcs(Q.accb, e);
+  const float2 chi0 = __ldcg(&Q.chi0[e]);   // written by this CTA earlier in the launch: L2, not the
+  const float2 dschi = __ldcg(&Q.dsch[e]);  // read-only path
+  // kappa and the hyper-viscosity rate of this (kx, ky)
+  const float kap = -(pk * I.ksx + fmf * I.kcz);
+  const float pk2 = pk * pk, fm2 = fmf * fmf;
+  const float wc = wsd[2] + C.wv[2] - (I.hx4 * (pk2 * pk2) + I.hy4 * (fm2 * fm2));
+  float2 r = gkfft::cscale(wc, f0);
+  r = gkfft::caxpy(wsd[0], fs[0], r);
+  r = gkfft::caxpy(wsd[1], fs[1], r);
+  r = gkfft::caxpy(wsd[3], fs[3], r);
+  r = gkfft::caxpy(wsd[4], fs[4], r);
+  r = gkfft::caxpy(C.wv[0], fv0, r);
+  r = gkfft::caxpy(C.wv[1], fv1, r);
+  r = gkfft::caxpy(C.wv[3], fv3, r);
+  r = gkfft::caxpy(C.wv[4], fv4, r);
+  r = gkfft::caxpy(C.c7, dschi, r);
+  // -i a z = a (z.y, -z.x)
+  r = gkfft::caxpy(C.a2 * kap, make_float2(f0.y, -f0.x), r);
+  r = gkfft::caxpy(C.a5 * (fmf * P.ky0) + C.a8 * kap, make_float2(chi0.y, -chi0.x), r);
+  r = gkfft::caxpy(scale, nlv, r);
+  float2 out;
+  if constexpr (MODE == 0) {
+    out = r;
+  } else if constexpr (MODE == 1) {
+    Cv<ST>::stcs(Q.accb, e, gkfft::caxpy(A.b, r, f0));
+    out = gkfft::caxpy(A.c, r, f0);
+  } else if constexpr (MODE == 2) {
+    Cv<ST>::stcs(Q.accb, e, gkfft::caxpy(A.b, r, ac));
+    out = gkfft::caxpy(A.c, r, fn);
+  } else {
+    out = gkfft::caxpy(A.b, r, ac);
+  }
+  Cv<ST>::stcs(Q.outb, e, out);
+  return out;
+}
+
+// chi = J0 phi and its parallel derivative for both streaming directions (VII), into the per-CTA
+// scratch `chis` (chi0, D_s chi for v>0, D_s chi for v<0)
+__device__ __forceinline__ void build_chis(const GkDev &P, const GkStageArgs &A, int a, int l, int i,
+                                           int slab, int nky, float2 *chis, int tid, int nthr) {
+  const long long jb = (((long long)a * P.nmu + l) * P.ns + i) * P.slab;
+  const float2 *ph = A.phi + (long long)i * P.slab;
+  for (int e = tid; e < slab; e += nthr) {
+    const int ip = e / nky, m = e - ip * nky;
+    const int cls = stencil_class(P, i, ip, m);
+    float2 c0 = make_float2(0.f, 0.f), dp = c0, dn = c0;
+#pragma unroll
+    for (int d = 0; d < 5; ++d) {
+      int off;
+      if (!seam_offset(P, i, d - 2, ip, m, off)) continue;
+      const float j0 = __ldg(&P.J0[jb + e + off]);
+      const float2 ph0 = __ldg(&ph[e + off]);
+      const float2 ch = make_float2(j0 * ph0.x, j0 * ph0.y);
+      if (d == 2) c0 = ch;
+      dp.x += P.dcoef[cls][0][d] * ch.x; dp.y += P.dcoef[cls][0][d] * ch.y;
+      dn.x += P.dcoef[cls][1][d] * ch.x; dn.y += P.dcoef[cls][1][d] * ch.y;
+    }
+    chis[e] = c0;
+    chis[slab + e] = dp;
+    chis[2 * slab + e] = dn;
+  }
+}
+
 // =================================================================================================
 // NT threads per CTA, OCC resident CTAs per SM (OCC = 2: grad(chi) is kept in the per-CTA global
 // scratch so that two CTAs fit one SM and their memory-bound and FFT phases overlap).
@@ -222,28 +341,7 @@ gk_stage_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkStage
     ItemCtx I;
     make_item_ctx(P, a, l, i, I);
     {
-      // ---- chi = J0 phi and its parallel derivative for both streaming directions (VII) ----
-      const long long jb = (((long long)a * P.nmu + l) * P.ns + i) * P.slab;
-      const float2 *ph = A.phi + (long long)i * P.slab;
-      for (int e = tid; e < slab; e += nthr) {
-        const int ip = e / nky, m = e - ip * nky;
-        const int cls = stencil_class(P, i, ip, m);
-        float2 c0 = make_float2(0.f, 0.f), dp = c0, dn = c0;
-#pragma unroll
-        for (int d = 0; d < 5; ++d) {
-          int off;
-          if (!seam_offset(P, i, d - 2, ip, m, off)) continue;
-          const float j0 = __ldg(&P.J0[jb + e + off]);
-          const float2 p = __ldg(&ph[e + off]);
-          const float2 ch = make_float2(j0 * p.x, j0 * p.y);
-          if (d == 2) c0 = ch;
-          dp.x += P.dcoef[cls][0][d] * ch.x; dp.y += P.dcoef[cls][0][d] * ch.y;
-          dn.x += P.dcoef[cls][1][d] * ch.x; dn.y += P.dcoef[cls][1][d] * ch.y;
-        }
-        chis[e] = c0;
-        chis[slab + e] = dp;
-        chis[2 * slab + e] = dn;
-      }
+      build_chis(P, A, a, l, i, slab, nky, chis, tid, nthr);
       __syncthreads();
       if constexpr (NL) {
         to_real([&](int e) { return chis[e]; },
@@ -265,6 +363,19 @@ gk_stage_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkStage
       make_slab_ctx(P, I, j, C);
       const ST *yb = (const ST *)A.y + C.base;
       if constexpr (NL) {
+        // L2 prefetch of what the epilogue will read from HBM for the first time (the slab j+2 of
+        // the state, f_n and the accumulator of this slab): their latency hides behind the FFTs
+        if (P.prefetch) {
+          const int nline = (slab * (int)sizeof(ST) + 127) / 128;
+          if (tid < nline) {
+            const char *p0 = (const char *)(yb + C.ov[3]) + tid * 128;
+            const char *p1 = (const char *)((const ST *)A.fn + C.base) + tid * 128;
+            const char *p2 = (const char *)((const ST *)A.acc + C.base) + tid * 128;
+            if (C.ov[3] != 0) asm volatile("prefetch.global.L2 [%0];" ::"l"(p0));
+            if (A.mode == 2) asm volatile("prefetch.global.L2 [%0];" ::"l"(p1));
+            if (A.mode >= 2) asm volatile("prefetch.global.L2 [%0];" ::"l"(p2));
+          }
+        }
         to_real([&](int e) { return Cv<ST>::ldg(yb, e); },
                 [&](int r0) {
                   // bracket d_y chi d_x f - d_x chi d_y f, rows (p, p+rc/2) packed as (re, im), evaluated
@@ -327,79 +438,16 @@ gk_stage_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkStage
       // ---- epilogue: linear terms + bracket + RK update, one coalesced pass over the slab ----
       // The operands (own value, 4 parallel and 4 vpar neighbours, f_n, accumulator, chi, D_s chi)
       // are all requested before the arithmetic; the arithmetic is one packed-fp32 FMA per operand.
-      const ST *yv0 = yb + C.ov[0], *yv1 = yb + C.ov[1], *yv3 = yb + C.ov[2], *yv4 = yb + C.ov[3];
-      const ST *fnb = (const ST *)A.fn + C.base;
-      ST *accb = (ST *)A.acc + C.base, *outb = (ST *)A.out + C.base;
-      const float2 *dsch = chis + (1 + C.sg) * slab;
+      EpiPtrs<ST> Q;
+      make_epi_ptrs<ST>(A, C, chis, slab, Q);
       auto point = [&](auto modec, auto intc, int e, int ip, int m, float pk, float fmf) -> float2 {
-        constexpr int MODE = decltype(modec)::value;
-        constexpr bool INTERIOR = decltype(intc)::value != 0;
-        const float2 f0 = Cv<ST>::ldg(yb, e);
-        float2 fs[5];
-        float wsd[5];
-        if constexpr (INTERIOR) {
-          fs[0] = Cv<ST>::ldg(yb, e - 2 * slab);
-          fs[1] = Cv<ST>::ldg(yb, e - slab);
-          fs[3] = Cv<ST>::ldg(yb, e + slab);
-          fs[4] = Cv<ST>::ldg(yb, e + 2 * slab);
-#pragma unroll
-          for (int d = 0; d < 5; ++d) wsd[d] = C.ws[d];
-        } else {
-          const int cls = stencil_class(P, i, ip, m);
-#pragma unroll
-          for (int d = 0; d < 5; ++d) {
-            const float wgt = C.cI * P.dcoef[cls][C.sg][d] + C.cDs * P.discoef[cls][d];
-            if (d == 2) { wsd[d] = wgt; continue; }
-            int off;
-            const bool ok = seam_offset(P, i, d - 2, ip, m, off);
-            fs[d] = Cv<ST>::ldg(yb, e + off);
-            wsd[d] = ok ? wgt : 0.f;
-          }
-        }
-        const float2 fv0 = Cv<ST>::ldg(yv0, e), fv1 = Cv<ST>::ldg(yv1, e);
-        const float2 fv3 = Cv<ST>::ldg(yv3, e), fv4 = Cv<ST>::ldg(yv4, e);
-        float2 fn = f0, ac = make_float2(0.f, 0.f);
-        if constexpr (MODE == 2) fn = Cv<ST>::ldcs(fnb, e);
-        if constexpr (MODE >= 2) ac = Cv<ST>::ldcs(accb, e);
-        const float2 chi0 = chis[e];
-        const float2 dschi = dsch[e];
         float2 nlv = make_float2(0.f, 0.f);
         if constexpr (NL) {
           const int n = (ip >= K) ? ip - K : mx + ip - K;
           nlv = SA[n * ldx + m];
         }
-        // kappa and the hyper-viscosity rate of this (kx, ky)
-        const float kap = -(pk * I.ksx + fmf * I.kcz);
-        const float pk2 = pk * pk, fm2 = fmf * fmf;
-        const float wc = wsd[2] + C.wv[2] - (I.hx4 * (pk2 * pk2) + I.hy4 * (fm2 * fm2));
-        float2 r = gkfft::cscale(wc, f0);
-        r = gkfft::caxpy(wsd[0], fs[0], r);
-        r = gkfft::caxpy(wsd[1], fs[1], r);
-        r = gkfft::caxpy(wsd[3], fs[3], r);
-        r = gkfft::caxpy(wsd[4], fs[4], r);
-        r = gkfft::caxpy(C.wv[0], fv0, r);
-        r = gkfft::caxpy(C.wv[1], fv1, r);
-        r = gkfft::caxpy(C.wv[3], fv3, r);
-        r = gkfft::caxpy(C.wv[4], fv4, r);
-        r = gkfft::caxpy(C.c7, dschi, r);
-        // -i a z = a (z.y, -z.x)
-        r = gkfft::caxpy(C.a2 * kap, make_float2(f0.y, -f0.x), r);
-        r = gkfft::caxpy(C.a5 * (fmf * P.ky0) + C.a8 * kap, make_float2(chi0.y, -chi0.x), r);
-        if constexpr (NL) r = gkfft::caxpy(scale, nlv, r);
-        float2 out;
-        if constexpr (MODE == 0) {
-          out = r;
-        } else if constexpr (MODE == 1) {
-          Cv<ST>::stcs(accb, e, gkfft::caxpy(A.b, r, f0));
-          out = gkfft::caxpy(A.c, r, f0);
-        } else if constexpr (MODE == 2) {
-          Cv<ST>::stcs(accb, e, gkfft::caxpy(A.b, r, ac));
-          out = gkfft::caxpy(A.c, r, fn);
-        } else {
-          out = gkfft::caxpy(A.b, r, ac);
-        }
-        Cv<ST>::stcs(outb, e, out);
-        return out;
+        return rhs_point<ST, decltype(modec)::value, decltype(intc)::value != 0>(
+            P, A, I, C, Q, slab, e, ip, m, pk, fmf, nlv, scale);
       };
       auto epilogue = [&](auto modec, auto intc) {
         if constexpr (ROWMAP) {
