@@ -21,7 +21,7 @@ UNITS = [
     ("gk_stage_inst.cu", ["-DGK_ST_ID=1"], "gk_stage_f16.o"),
     ("gk_stage_inst.cu", ["-DGK_ST_ID=2"], "gk_stage_bf16.o"),
 ]
-DEPS = ["gk_lib.cu", "gk_stage_inst.cu", "gk_kernels.cuh", "gk_common.cuh", "gk_stage.cuh", "gk_stage_ws.cuh", "gk_fft.cuh", "gk_tables.h",
+DEPS = ["gk_lib.cu", "gk_stage_inst.cu", "gk_kernels.cuh", "gk_common.cuh", "gk_stage.cuh", "gk_stage_ws.cuh", "gk_stage_ws2.cuh", "gk_fft.cuh", "gk_tables.h",
         "gk_dev.h", "gk_pick.h"]
 
 NVCC_FLAGS = [

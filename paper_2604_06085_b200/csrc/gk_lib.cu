@@ -288,7 +288,12 @@ int gk_create(const gk_grid *g, const gk_species *sp, const gk_salpha *geo, cons
     nwork = (long long)T.nsp * T.nmu * T.ns * P.nchunk;
 
     // shared-memory plan (per CTA: the SM's 227 KB opt-in capacity / occ, minus 1 KB reserved per CTA)
-    if (nl) {
+    if (nl && pick.smem) {  // in-place warp-specialised kernel: fixed plan
+      P.rc = P.mx;
+      P.gchi_in_smem = 1;
+      c->stage_smem = pick.smem;
+      c->stage_grid = (int)std::min<long long>(nwork, resident);
+    } else if (nl) {
       const size_t cap = pick.occ == 1 ? kSmemMax : (kSmemMax + 1024) / pick.occ - 1024;
       const size_t fixed = ((size_t)P.mx + P.my + (size_t)P.mx * P.ldx) * 8;
       const size_t gbytes = (size_t)P.mx * P.ldy * 8;

@@ -3,6 +3,7 @@
 #include "gk_common.cuh"
 #include "gk_stage.cuh"
 #include "gk_stage_ws.cuh"
+#include "gk_stage_ws2.cuh"
 #include "gk_pick.h"
 
 #ifndef GK_ST_ID
@@ -27,7 +28,7 @@ namespace {
 template <class ST> StagePick pick_stage(int mx, int my, int nky, int nkx, bool nl, int want_occ, int want_thr) {
 #define GK_SPEC(MX, MY, NKY, NKX, NT, OCC)                                                       \
   if (nl && mx == MX && my == MY && nky == NKY && nkx == NKX && want_occ == OCC && want_thr == NT) \
-    return {(const void *)gk::gk_stage_kernel<ST, MX, MY, NKY, NKX, true, NT, OCC>, NT, OCC, 0}
+    return {(const void *)gk::gk_stage_kernel<ST, MX, MY, NKY, NKX, true, NT, OCC>, NT, OCC, 0, 0}
   GK_SPEC(16, 12, 4, 9, 512, 1);
   GK_SPEC(128, 48, 16, 85, 1024, 1);
   GK_SPEC(128, 48, 16, 85, 512, 2);
@@ -40,29 +41,49 @@ template <class ST> StagePick pick_stage(int mx, int my, int nky, int nkx, bool 
   // term III switched off: a streaming stencil kernel
 #define GK_SPEC_LIN(NKY, NKX)                                                                    \
   if (!nl && nky == NKY && nkx == NKX && want_occ == 1 && want_thr == 1024)                      \
-    return {(const void *)gk::gk_stage_kernel<ST, 0, 0, NKY, NKX, false, 1024, 1>, 1024, 1, 0}
+    return {(const void *)gk::gk_stage_kernel<ST, 0, 0, NKY, NKX, false, 1024, 1>, 1024, 1, 0, 0}
   GK_SPEC_LIN(16, 85);
   GK_SPEC_LIN(32, 85);
   GK_SPEC_LIN(64, 127);
 #undef GK_SPEC_LIN
-  return {nullptr, 0, 0, 0};
+  return {nullptr, 0, 0, 0, 0};
 }
 // preference order of (threads, occ) variants; the first one that exists and fits is used
 // warp-specialised variants (FFT-role threads, epilogue-role threads)
 template <class ST> StagePick pick_stage_ws(int mx, int my, int nky, int nkx, int ntf) {
 #define GK_WS(MX, MY, NKY, NKX, NTF, NTE)                                         \
   if (mx == MX && my == MY && nky == NKY && nkx == NKX && ntf == NTF)             \
-    return {(const void *)gk::gk_stage_ws_kernel<ST, MX, MY, NKY, NKX, NTF, NTE>, NTF + NTE, 1, NTF}
+    return {(const void *)gk::gk_stage_ws_kernel<ST, MX, MY, NKY, NKX, NTF, NTE>, NTF + NTE, 1, NTF, 0}
   GK_WS(128, 48, 16, 85, 512, 512);
   GK_WS(128, 96, 32, 85, 512, 512);
   GK_WS(128, 96, 32, 85, 768, 256);
   GK_WS(192, 192, 64, 127, 512, 512);
 #undef GK_WS
-  return {nullptr, 0, 0, 0};
+  return {nullptr, 0, 0, 0, 0};
+}
+// in-place variants (gk_stage_ws2_kernel): the padded field and grad(chi) both live in shared memory.
+// `code` = FFT-role threads, +1, +2, ... for the alternative role splits (GK_WS_NTF, tuning).
+template <class ST> StagePick pick_stage_ws2(int mx, int my, int nky, int nkx, int code) {
+#define GK_WS2(CODE, MX, MY, NKY, NKX, NTF, NTE, RF, RE, NB)                      \
+  if (mx == MX && my == MY && nky == NKY && nkx == NKX && code == CODE)           \
+    return {(const void *)gk::gk_stage_ws2_kernel<ST, MX, MY, NKY, NKX, NTF, NTE, RF, RE, NB>, NTF + NTE, 1, NTF, \
+            gk::ws2_smem_bytes<ST, MX, MY, NKY, NKX>()}
+  GK_WS2(512, 128, 96, 32, 85, 512, 256, 56, 128, 2);
+  GK_WS2(513, 128, 96, 32, 85, 512, 512, 0, 0, 1);
+  GK_WS2(514, 128, 96, 32, 85, 512, 384, 56, 88, 1);
+  GK_WS2(515, 128, 96, 32, 85, 512, 384, 56, 88, 2);
+  GK_WS2(516, 128, 96, 32, 85, 512, 256, 56, 128, 3);
+  GK_WS2(512, 128, 48, 16, 85, 512, 256, 56, 128, 2);
+#undef GK_WS2
+  return {nullptr, 0, 0, 0, 0};
 }
 template <class ST> StagePick pick_stage_auto(int mx, int my, int nky, int nkx, bool nl, int force_occ, int force_thr, int ws_ntf) {
+  const bool ws_old = ws_ntf < 0;  // negative: the chunked warp-specialised kernel (gk_stage_ws_kernel)
+  if (ws_old) ws_ntf = -ws_ntf;
   if (nl && ws_ntf > 0) {
-    StagePick p = pick_stage_ws<ST>(mx, my, nky, nkx, ws_ntf);
+    StagePick p = ws_old ? StagePick{nullptr, 0, 0, 0, 0} : pick_stage_ws2<ST>(mx, my, nky, nkx, ws_ntf);
+    if (p.fn) return p;
+    p = pick_stage_ws<ST>(mx, my, nky, nkx, ws_ntf);
     if (p.fn) return p;
   }
   static const int pref[][2] = {{1024, 1}, {512, 2}, {512, 1}};
@@ -72,8 +93,8 @@ template <class ST> StagePick pick_stage_auto(int mx, int my, int nky, int nkx, 
     StagePick p = pick_stage<ST>(mx, my, nky, nkx, nl, pr[1], pr[0]);
     if (p.fn) return p;
   }
-  if (!nl) return {(const void *)gk::gk_stage_kernel<ST, 0, 0, 0, 0, false, 512, 1>, 512, 1, 0};
-  return {(const void *)gk::gk_stage_kernel<ST, 0, 0, 0, 0, true, 512, 1>, 512, 1, 0};
+  if (!nl) return {(const void *)gk::gk_stage_kernel<ST, 0, 0, 0, 0, false, 512, 1>, 512, 1, 0, 0};
+  return {(const void *)gk::gk_stage_kernel<ST, 0, 0, 0, 0, true, 512, 1>, 512, 1, 0, 0};
 }
 
 

@@ -26,6 +26,98 @@ __device__ __forceinline__ void bar_arrive_n(int id, int n) {
 
 #define GK_WS_CHI_RING 3
 #define GK_WS_NL_RING 2
+#define GK_WS_BAR_FFT 1
+#define GK_WS_BAR_FULL 2
+#define GK_WS_BAR_FREE 4
+
+// Epilogue role of the warp-specialised kernels: linear terms + RK update + moment of slab u once the
+// FFT role has published its bracket in ring slot u & 1 (BAR_FULL), then releases the slot (BAR_FREE).
+template <class ST, int NKY_, int NKX_, int NTF, int NTE>
+__device__ __forceinline__ void ws_epilogue_role(const GkDev &P, const GkStageArgs &A, const float2 *chis_cta,
+                                                 const float2 *nl_cta, int tid) {
+  constexpr int NT = NTF + NTE;
+  constexpr int nky = NKY_, nkx = NKX_;
+  constexpr int K = (nkx - 1) / 2, slab = nkx * nky;
+  constexpr int BAR_FULL = GK_WS_BAR_FULL, BAR_FREE = GK_WS_BAR_FREE;
+  static_assert(NTE % NKY_ == 0, "an epilogue sweep covers whole ky rows");
+  // =============================== epilogue role ================================
+  const int et = tid - NTF;
+  constexpr int EPT = (slab + NTE - 1) / NTE;
+  constexpr int RS = NTE / nky;  // kx rows per sweep of the role's threads
+  const int m = et % nky, ip0 = et / nky;
+  const float fmf = (float)m, pk0 = (float)(ip0 - K);
+  const float scale = 0.25f * P.fftnorm;  // 1/2 (bracket) * 1/2 (two-for-one unpack) / (mx my)
+  int u = 0, it = 0;
+  for (int w = blockIdx.x; w < A.nwork; w += gridDim.x, ++it) {
+    const int i = w % P.ns;
+    const int c = (w / P.ns) % P.nchunk;
+    const int al = w / (P.ns * P.nchunk);
+    const int l = al % P.nmu, a = al / P.nmu;
+    ItemCtx I;
+    make_item_ctx(P, a, l, i, I);
+    const float2 *chis = chis_cta + (it % GK_WS_CHI_RING) * 3 * slab;
+    float2 macc[EPT];
+#pragma unroll
+    for (int k = 0; k < EPT; ++k) macc[k] = make_float2(0.f, 0.f);
+    const bool interior = (i >= 2 && i < P.ns - 2);
+    const int j1 = min(P.nv, (c + 1) * P.jchunk);
+    for (int j = c * P.jchunk; j < j1; ++j, ++u) {
+      SlabCtx C;
+      make_slab_ctx(P, I, j, C);
+      EpiPtrs<ST> Q;
+      make_epi_ptrs<ST>(A, C, chis, slab, Q);
+      // L2 prefetch of what the NEXT slab reads from HBM for the first time (slab j+3 of the
+      // state, f_n and the accumulator of slab j+1)
+      if (P.prefetch && j + 1 < j1) {
+        constexpr int nline = (slab * (int)sizeof(ST) + 127) / 128;
+        for (int t = et; t < nline; t += NTE) {
+          const long long nb = C.base + I.jstride;
+          if (j + 3 < P.nv) asm volatile("prefetch.global.L2 [%0];" ::"l"((const char *)(Q.yb + 3 * I.jstride) + t * 128));
+          if (A.mode == 2) asm volatile("prefetch.global.L2 [%0];" ::"l"((const char *)((const ST *)A.fn + nb) + t * 128));
+          if (A.mode >= 2) asm volatile("prefetch.global.L2 [%0];" ::"l"((const char *)((const ST *)A.acc + nb) + t * 128));
+        }
+      }
+      const float2 *nlr = nl_cta + (u & 1) * slab;
+      bar_sync_n(BAR_FULL + (u & 1), NT);
+      auto sweep = [&](auto modec, auto intc) {
+#pragma unroll
+        for (int k = 0; k < EPT; ++k) {
+          const int e = et + k * NTE;
+          if (k + 1 < EPT || e < slab) {
+            const float2 out = rhs_point<ST, decltype(modec)::value, decltype(intc)::value != 0>(
+                P, A, I, C, Q, slab, e, ip0 + k * RS, m, pk0 + (float)(k * RS), fmf, __ldcg(&nlr[e]), scale);
+            macc[k] = cadd(macc[k], out);
+            // one point's 13 operands in flight per thread is all the registers allow: keep the
+            // compiler from hoisting the next point's loads above this one's arithmetic
+            asm volatile("" ::: "memory");
+          }
+        }
+      };
+      auto by_plane = [&](auto modec) {
+        if (interior) sweep(modec, gkfft::IC<1>{});
+        else sweep(modec, gkfft::IC<0>{});
+      };
+      switch (A.mode) {
+        case 0: by_plane(gkfft::IC<0>{}); break;
+        case 1: by_plane(gkfft::IC<1>{}); break;
+        case 2: by_plane(gkfft::IC<2>{}); break;
+        default: by_plane(gkfft::IC<3>{}); break;
+      }
+      bar_arrive_n(BAR_FREE + (u & 1), NT);
+    }
+    if (A.mom) {
+      // moment plane of this item: Z n 2 pi w_v B_i w_mu J0 sum_j f   (a1 of the next stage)
+      const float momw = P.sp[a].momfac * P.wmu[l] * P.B[i];
+      const float *j0p = P.J0 + (((long long)a * P.nmu + l) * P.ns + i) * P.slab;
+      float2 *dst = A.mom + (((long long)a * P.nmu + l) * P.nchunk + c) * P.nphi + (long long)i * P.slab;
+#pragma unroll
+      for (int k = 0; k < EPT; ++k) {
+        const int e = et + k * NTE;
+        if (e < slab) dst[e] = gkfft::cscale(momw * __ldg(&j0p[e]), macc[k]);
+      }
+    }
+  }
+}
 
 template <class ST, int MX_, int MY_, int NKY_, int NKX_, int NTF, int NTE>
 __global__ void __launch_bounds__(NTF + NTE, 1)
@@ -37,7 +129,7 @@ gk_stage_ws_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkSt
   constexpr int ldx = 2 * nky + 1, ldy = my | 1;
   static_assert(NTF % 32 == 0 && NTE % 32 == 0, "roles are whole warps");
   static_assert(NTE % NKY_ == 0, "an epilogue sweep covers whole ky rows");
-  constexpr int BAR_FFT = 1, BAR_FULL = 2, BAR_FREE = 4;
+  constexpr int BAR_FFT = GK_WS_BAR_FFT, BAR_FULL = GK_WS_BAR_FULL, BAR_FREE = GK_WS_BAR_FREE;
   const int tid = threadIdx.x;
   float2 *chis_cta = A.chis + (long long)blockIdx.x * (GK_WS_CHI_RING * 3 * slab);
   float2 *nl_cta = A.nlbuf + (long long)blockIdx.x * (GK_WS_NL_RING * slab);
@@ -203,83 +295,7 @@ gk_stage_ws_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkSt
     // consume the epilogue's last arrivals so that no barrier is left half-way at exit
     for (int v = max(0, u - GK_WS_NL_RING); v < u; ++v) bar_sync_n(BAR_FREE + (v & 1), NT);
   } else {
-    // =============================== epilogue role ================================
-    const int et = tid - NTF;
-    constexpr int EPT = (slab + NTE - 1) / NTE;
-    constexpr int RS = NTE / nky;  // kx rows per sweep of the role's threads
-    const int m = et % nky, ip0 = et / nky;
-    const float fmf = (float)m, pk0 = (float)(ip0 - K);
-    const float scale = 0.25f * P.fftnorm;  // 1/2 (bracket) * 1/2 (two-for-one unpack) / (mx my)
-    int u = 0, it = 0;
-    for (int w = blockIdx.x; w < A.nwork; w += gridDim.x, ++it) {
-      const int i = w % P.ns;
-      const int c = (w / P.ns) % P.nchunk;
-      const int al = w / (P.ns * P.nchunk);
-      const int l = al % P.nmu, a = al / P.nmu;
-      ItemCtx I;
-      make_item_ctx(P, a, l, i, I);
-      const float2 *chis = chis_cta + (it % GK_WS_CHI_RING) * 3 * slab;
-      float2 macc[EPT];
-#pragma unroll
-      for (int k = 0; k < EPT; ++k) macc[k] = make_float2(0.f, 0.f);
-      const bool interior = (i >= 2 && i < P.ns - 2);
-      const int j1 = min(P.nv, (c + 1) * P.jchunk);
-      for (int j = c * P.jchunk; j < j1; ++j, ++u) {
-        SlabCtx C;
-        make_slab_ctx(P, I, j, C);
-        EpiPtrs<ST> Q;
-        make_epi_ptrs<ST>(A, C, chis, slab, Q);
-        // L2 prefetch of what the NEXT slab reads from HBM for the first time (slab j+3 of the
-        // state, f_n and the accumulator of slab j+1)
-        if (P.prefetch && j + 1 < j1) {
-          constexpr int nline = (slab * (int)sizeof(ST) + 127) / 128;
-          for (int t = et; t < nline; t += NTE) {
-            const long long nb = C.base + I.jstride;
-            if (j + 3 < P.nv) asm volatile("prefetch.global.L2 [%0];" ::"l"((const char *)(Q.yb + 3 * I.jstride) + t * 128));
-            if (A.mode == 2) asm volatile("prefetch.global.L2 [%0];" ::"l"((const char *)((const ST *)A.fn + nb) + t * 128));
-            if (A.mode >= 2) asm volatile("prefetch.global.L2 [%0];" ::"l"((const char *)((const ST *)A.acc + nb) + t * 128));
-          }
-        }
-        const float2 *nlr = nl_cta + (u & 1) * slab;
-        bar_sync_n(BAR_FULL + (u & 1), NT);
-        auto sweep = [&](auto modec, auto intc) {
-#pragma unroll
-          for (int k = 0; k < EPT; ++k) {
-            const int e = et + k * NTE;
-            if (k + 1 < EPT || e < slab) {
-              const float2 out = rhs_point<ST, decltype(modec)::value, decltype(intc)::value != 0>(
-                  P, A, I, C, Q, slab, e, ip0 + k * RS, m, pk0 + (float)(k * RS), fmf, __ldcg(&nlr[e]), scale);
-              macc[k] = cadd(macc[k], out);
-              // one point's 13 operands in flight per thread is all the registers allow: keep the
-              // compiler from hoisting the next point's loads above this one's arithmetic
-              asm volatile("" ::: "memory");
-            }
-          }
-        };
-        auto by_plane = [&](auto modec) {
-          if (interior) sweep(modec, gkfft::IC<1>{});
-          else sweep(modec, gkfft::IC<0>{});
-        };
-        switch (A.mode) {
-          case 0: by_plane(gkfft::IC<0>{}); break;
-          case 1: by_plane(gkfft::IC<1>{}); break;
-          case 2: by_plane(gkfft::IC<2>{}); break;
-          default: by_plane(gkfft::IC<3>{}); break;
-        }
-        bar_arrive_n(BAR_FREE + (u & 1), NT);
-      }
-      if (A.mom) {
-        // moment plane of this item: Z n 2 pi w_v B_i w_mu J0 sum_j f   (a1 of the next stage)
-        const float momw = P.sp[a].momfac * P.wmu[l] * P.B[i];
-        const float *j0p = P.J0 + (((long long)a * P.nmu + l) * P.ns + i) * P.slab;
-        float2 *dst = A.mom + (((long long)a * P.nmu + l) * P.nchunk + c) * P.nphi + (long long)i * P.slab;
-#pragma unroll
-        for (int k = 0; k < EPT; ++k) {
-          const int e = et + k * NTE;
-          if (e < slab) dst[e] = gkfft::cscale(momw * __ldg(&j0p[e]), macc[k]);
-        }
-      }
-    }
+    ws_epilogue_role<ST, NKY_, NKX_, NTF, NTE>(P, A, chis_cta, nl_cta, tid);
   }
 }
 
