@@ -52,43 +52,57 @@ def _traffic(workload):
 
 
 class ClockSampler:
-    """nvidia-smi clocks and throttle reasons sampled DURING the timed region."""
+    """nvidia-smi clocks and throttle reasons sampled DURING the timed region: start() returns once the
+    first sample has arrived, mark() brackets the timed region on the host clock, stop() reports the
+    samples that fall inside the marks (all samples of the run if the region was shorter than one
+    sampling period, said so in `window`)."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
 
     def __init__(self, index: int):
-        self.rows, self.proc, self.index = [], None, index
+        self.rows, self.proc, self.index, self.marks = [], None, index, []
 
     def start(self):
         try:
             self.proc = subprocess.Popen(
                 ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                 "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+                 "-lms", "25"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.th = threading.Thread(target=self._read, daemon=True)
             self.th.start()
+            t0 = time.perf_counter()
+            while not self.rows and time.perf_counter() - t0 < 5.0:
+                time.sleep(0.01)
         except Exception:
             self.proc = None
 
     def _read(self):
         for line in self.proc.stdout:
-            self.rows.append([x.strip() for x in line.split(",")])
+            self.rows.append((time.perf_counter(), [x.strip() for x in line.split(",")]))
+
+    def mark(self):
+        self.marks.append(time.perf_counter())
 
     def stop(self):
         if not self.proc:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        time.sleep(0.15)
+        time.sleep(0.05)
         self.proc.terminate()
-        sm = [float(r[0]) for r in self.rows if r and r[0].replace(".", "").isdigit()]
-        mx = [float(r[1]) for r in self.rows if len(r) > 1 and r[1].replace(".", "").isdigit()]
+        rows, window = [r for _, r in self.rows], "whole run"
+        if len(self.marks) >= 2:
+            inside = [r for t, r in self.rows if self.marks[0] <= t <= self.marks[-1] + 0.03]
+            if inside:
+                rows, window = inside, "timed region"
+        sm = [float(r[0]) for r in rows if r and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in rows if len(r) > 1 and r[1].replace(".", "").isdigit()]
         reasons = set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for r in self.rows:
+        for r in rows:
             for k, n in enumerate(names):
                 if len(r) > 3 + k and r[3 + k].lower().startswith("active"):
                     reasons.add(n)
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "reasons": sorted(reasons), "samples": len(sm)}
+                "reasons": sorted(reasons), "samples": len(sm), "window": window}
 
 
 def _oracle_sample(cfg, budget_s=15.0):
@@ -228,10 +242,12 @@ def main():
     g.gk_stage_kernel_time(reset=True)
     l0 = g.gk_launch_count()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sampler.mark()
     e0.record()
     g.gk_rk4_steps(fd, dt, args.steps)
     e1.record()
     barrier()
+    sampler.mark()
     ms = e0.elapsed_time(e1)
     launches = g.gk_launch_count() - l0
     stage_ms, stage_n = g.gk_stage_kernel_time(reset=True)
@@ -288,7 +304,7 @@ def main():
             "gpu_launches": int(launches),
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
                          "frac": achieved / peak, "traffic": _traffic(cfg["name"]), "peak_source": peak_src,
-                         "kernel": "gk_stage_kernel", "launches_timed": int(stage_n),
+                         "kernel": {0: "gk_stage_kernel"}.get(plan.get("ws", 0), "gk_stage_ws2_kernel" if plan.get("rc") == plan.get("mx") else "gk_stage_ws_kernel"), "launches_timed": int(stage_n),
                          "avg_launch_ms": stage_avg_ms, "alg_bytes_per_point": bpp,
                          "stage_share_of_step": stage_ms / ms if ms > 0 else None},
         }
