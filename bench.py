@@ -304,7 +304,7 @@ def main():
             "gpu_launches": int(launches),
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
                          "frac": achieved / peak, "traffic": _traffic(cfg["name"]), "peak_source": peak_src,
-                         "kernel": {0: "gk_stage_kernel"}.get(plan.get("ws", 0), "gk_stage_ws2_kernel" if plan.get("rc") == plan.get("mx") else "gk_stage_ws_kernel"), "launches_timed": int(stage_n),
+                         "kernel": ["gk_stage_kernel", "gk_stage_ws_kernel", "gk_stage_ws2_kernel", "gk_stage_lin_kernel"][plan.get("kind", 0)], "launches_timed": int(stage_n),
                          "avg_launch_ms": stage_avg_ms, "alg_bytes_per_point": bpp,
                          "stage_share_of_step": stage_ms / ms if ms > 0 else None},
         }

@@ -37,7 +37,7 @@ struct gk_ctx {
   bool poisoned = false;
   int num_sms = 0;
   int stage_grid = 0;
-  int stage_threads = 512, stage_occ = 1, stage_ws = 0;
+  int stage_threads = 512, stage_occ = 1, stage_ws = 0, stage_kind = 0;
   size_t stage_smem = 0;
   size_t elem_bytes = 8;
   // workspace
@@ -267,6 +267,7 @@ int gk_create(const gk_grid *g, const gk_species *sp, const gk_salpha *geo, cons
     c->stage_threads = pick.threads;
     c->stage_occ = pick.occ;
     c->stage_ws = pick.ws;
+    c->stage_kind = pick.kind;
     const int resident = c->num_sms * pick.occ;  // persistent CTAs
 
     // work decomposition: items (a, l, vpar chunk, i) are dealt round-robin to the persistent CTAs.
@@ -320,7 +321,7 @@ int gk_create(const gk_grid *g, const gk_species *sp, const gk_salpha *geo, cons
     } else {
       P.rc = 2;
       P.gchi_in_smem = 1;
-      c->stage_smem = (size_t)P.slab * 8;
+      c->stage_smem = pick.kind == 3 ? 0 : (size_t)P.slab * 8;
       c->stage_grid = (int)std::min<long long>(nwork, resident);
     }
     break;
@@ -497,7 +498,7 @@ size_t gk_export_table(const gk_ctx *c, const char *which, double *out, size_t m
   } else if (w == "pad") {
     tmp = {(double)c->P.mx, (double)c->P.my, (double)c->P.rc, (double)c->P.gchi_in_smem,
            (double)c->P.jchunk, (double)c->P.nchunk, (double)c->stage_grid, (double)c->stage_smem,
-           (double)c->stage_threads, (double)c->stage_occ, (double)c->stage_ws};
+           (double)c->stage_threads, (double)c->stage_occ, (double)c->stage_ws, (double)c->stage_kind};
     src = &tmp;
   } else return 0;
   if (out) std::memcpy(out, src->data(), std::min(maxn, src->size()) * sizeof(double));

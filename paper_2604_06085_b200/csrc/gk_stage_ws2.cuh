@@ -86,9 +86,10 @@ constexpr size_t ws2_smem_bytes() {
 // (open chain end: PAPER.md:350, 362; R7).
 
 template <class ST, int NKY_, int NKX_, int NTF, int NTE, int NB>
-__device__ __forceinline__ void ws_epilogue_role2(const GkDev &P, const GkStageArgs &A, const float2 *chis_cta,
+__device__ __forceinline__ void ws_epilogue_role2(const GkDev &P, const GkStageArgs &A, float2 *chis_cta,
                                                   const float2 *nl_cta, float *eblk, int tid) {
   constexpr int NT = NTF + NTE;
+  constexpr bool NL = NTF > 0;   // NTF == 0: the whole CTA runs this role and term III is off
   constexpr int nky = NKY_, nkx = NKX_;
   constexpr int K = (nkx - 1) / 2, slab = nkx * nky;
   constexpr int BAR_FULL = GK_WS_BAR_FULL, BAR_FREE = GK_WS_BAR_FREE;
@@ -110,6 +111,11 @@ __device__ __forceinline__ void ws_epilogue_role2(const GkDev &P, const GkStageA
     const int l = al % P.nmu, a = al / P.nmu;
     const long long base0 = (((long long)a * P.nv * P.nmu + l) * P.ns + i) * P.slab;
     const float2 *chip = chis_cta + (it % GK_WS_CHI_RING) * 3 * slab + et;
+    // without an FFT role the CTA builds chi and D_s chi itself; the first barrier below publishes them
+    if constexpr (!NL) {
+      build_chis(P, A, a, l, i, slab, nky, chis_cta + (it % GK_WS_CHI_RING) * 3 * slab, et, NTE);
+      bar_sync_n(BAR_FULL, NT);   // the only CTA-wide barrier of an item: warps march along vpar on their own
+    }
     // per item: kappa = -(pk ksx + m kcz), hyper-viscosity hx4 (p/K)^4 + hy4 (m/(nky-1))^4
     const int mask = P.mask;
     const float ksx = P.dkx * P.sth[i], kcz = P.ky0 * P.cz[i];
@@ -132,11 +138,13 @@ __device__ __forceinline__ void ws_epilogue_role2(const GkDev &P, const GkStageA
     for (int k = 0; k < EPT; ++k) macc[k] = make_float2(0.f, 0.f);
     const int j0 = c * P.jchunk, j1 = min(P.nv, (c + 1) * P.jchunk);
     for (int j = j0; j < j1; ++j, ++u) {
-      float *eb = eblk + (u & 1) * GK_EB_N;
+      // coefficient block: one per CTA and slab parity beside an FFT role (published by BAR_FULL), one per warp otherwise
+      float *eb = NL ? eblk + (u & 1) * GK_EB_N : eblk + (et >> 5) * GK_EB_N;
+      if constexpr (!NL) __syncwarp();
       const bool m2 = j >= 2, m1 = j >= 1, p1 = j + 1 < P.nv, p2 = j + 2 < P.nv;
       const float vj = P.v[j];
       const int sg = (vj > 0.f) ? 0 : 1;
-      if (et == 0) {  // slab-uniform coefficients, one thread
+      if (NL ? et == 0 : (et & 31) == 0) {  // slab-uniform coefficients, one thread
         const GkSpeciesDev &Sp = P.sp[a];
         const float mul = P.mu[l], muB = mul * P.B[i];
         const float E = vj * vj + 2.f * muB, ED = vj * vj + muB;
@@ -187,7 +195,8 @@ __device__ __forceinline__ void ws_epilogue_role2(const GkDev &P, const GkStageA
       }
       const float2 *nlr = nl_cta + (u & 1) * slab + et;
       const float2 *dsp = chip + (1 + sg) * slab;
-      bar_sync_n(BAR_FULL + (u & 1), NT);   // also publishes eb to the role's other threads
+      if constexpr (NL) bar_sync_n(BAR_FULL + (u & 1), NT);   // also publishes eb to the role's other threads
+      else __syncwarp();
       auto sweep = [&](auto modec, auto seamc) {
         constexpr int MODE = decltype(modec)::value;
         constexpr bool SEAM = decltype(seamc)::value != 0;
@@ -222,7 +231,23 @@ __device__ __forceinline__ void ws_epilogue_role2(const GkDev &P, const GkStageA
               if constexpr (MODE >= 2) ac[q] = Cv<ST>::ldcs(accp, eo);
               chi0[q] = __ldcg(chip + eo);    // written by this CTA earlier in the launch: L2, not the
               dschi[q] = __ldcg(dsp + eo);    // read-only path
-              nlv[q] = __ldcg(nlr + eo);
+              nlv[q] = make_float2(0.f, 0.f);
+              if constexpr (NL) nlv[q] = __ldcg(nlr + eo);
+            }
+          }
+          if constexpr (!NL) {  // no FFT role: shared memory is unused, L1 is large: next batch's operands -> L1
+#pragma unroll
+            for (int q = 0; q < NB; ++q) {
+              const int k = k0 + NB + q, eo = k * NTE;
+              if (k < EPT && (k + 1 < EPT || et + eo < slab)) {
+                int o0 = -2 * slab, o1 = -slab, o3 = slab, o4 = 2 * slab;
+                if constexpr (SEAM) { o0 = soff[0]; o1 = soff[1]; o3 = soff[2]; o4 = soff[3]; }
+                auto pf = [](const void *ptr) { asm volatile("prefetch.global.L1 [%0];" ::"l"(ptr)); };
+                pf(yp + eo); pf(yp + eo + o0); pf(yp + eo + o1); pf(yp + eo + o3); pf(yp + eo + o4);
+                pf(yp + eo + ov0); pf(yp + eo + ov1); pf(yp + eo + ov3); pf(yp + eo + ov4);
+                if constexpr (MODE == 2) pf(fnp + eo);
+                if constexpr (MODE >= 2) pf(accp + eo);
+              }
             }
           }
           asm volatile("" ::: "memory");      // coefficient loads stay behind the operand loads
@@ -253,7 +278,7 @@ __device__ __forceinline__ void ws_epilogue_role2(const GkDev &P, const GkStageA
               // -i a z = a (z.y, -z.x)
               r = gkfft::caxpy(we.x * kap, make_float2(f0[q].y, -f0[q].x), r);
               r = gkfft::caxpy(we.y * fmf + we.z * kap, make_float2(chi0[q].y, -chi0[q].x), r);
-              r = gkfft::caxpy(scale, nlv[q], r);
+              if constexpr (NL) r = gkfft::caxpy(scale, nlv[q], r);
               float2 out;
               if constexpr (MODE == 0) {
                 out = r;
@@ -283,7 +308,7 @@ __device__ __forceinline__ void ws_epilogue_role2(const GkDev &P, const GkStageA
         case 2: by_plane(gkfft::IC<2>{}); break;
         default: by_plane(gkfft::IC<3>{}); break;
       }
-      bar_arrive_n(BAR_FREE + (u & 1), NT);
+      if constexpr (NL) bar_arrive_n(BAR_FREE + (u & 1), NT);
     }
     if (A.mom) {
       // moment plane of this item: Z n 2 pi w_v B_i w_mu J0 sum_j f   (a1 of the next stage)
@@ -610,6 +635,17 @@ gk_stage_ws2_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkS
     if constexpr (RE > 0) asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(RE));
     ws_epilogue_role2<ST, NKY_, NKX_, NTF, NTE, NB>(P, A, chis_cta, nl_cta, eblk, tid);
   }
+}
+
+// Term III switched off: every thread of the CTA runs the lean epilogue (a streaming stencil + RK update);
+// OCC CTAs per SM, no FFT role, no dynamic shared memory.
+template <class ST, int NKY_, int NKX_, int NT, int NB, int OCC>
+__global__ void __launch_bounds__(NT, OCC)
+gk_stage_lin_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkStageArgs A) {
+  __shared__ __align__(16) float eblk[(NT / 32) * GK_EB_N];
+  constexpr int slab = NKX_ * NKY_;
+  float2 *chis_cta = A.chis + (long long)blockIdx.x * (GK_WS_CHI_RING * 3 * slab);
+  ws_epilogue_role2<ST, NKY_, NKX_, 0, NT, NB>(P, A, chis_cta, nullptr, eblk, threadIdx.x);
 }
 
 }  // namespace gk
