@@ -19,7 +19,7 @@
 //   XF1 forward x pass 1   the two-for-one unpack (Z(m), conj Z(my-m)) is done in its loads;
 //                          output to the dead columns nky..2nky-1
 //   XF2 forward x pass 2   retained kx -> the bracket ring in L2 for the epilogue role
-// Twiddles come from small shared tables laid out so that one 128-bit load yields two factors.
+// Twiddles come from compile-time tables in constant memory (warp-uniform indices).
 // Epilogue role: ws_epilogue_role of gk_stage_ws.cuh.
 #pragma once
 
@@ -59,23 +59,46 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
   }
 }
 
-// u[k] *= T[k] (S > 0) or conj T[k] (S < 0), k = 1..R-1; T is 16-byte aligned, two factors per load
+// Twiddle tables of the two-pass transforms N = R1 R2 in constant memory (compile-time initialised; warp-uniform
+// indices, so the loads go through the constant cache and not through the shared-memory/L1 data pipe that bounds
+// the kernel):  a[n1 R2 + k2] = b[k2 R1 + n1] = exp(+2 pi i n1 k2 / N)
+template <int N> struct TwTab { float2 a[N]; float2 b[N]; };
+template <int N> constexpr TwTab<N> make_tw() {
+  TwTab<N> t{};
+  constexpr int R1 = gkfft::Fac<N>::R1, R2 = gkfft::Fac<N>::R2;
+  for (int n1 = 0; n1 < R1; ++n1)
+    for (int k2 = 0; k2 < R2; ++k2) {
+      const int k = (n1 * k2) % N;
+      const double ang = 2.0 * gkfft::kPi * (k > N / 2 ? k - N : k) / N;
+      const float c = (float)gkfft::cx_cos(ang), sn = (float)gkfft::cx_sin(ang);
+      t.a[n1 * R2 + k2].x = c; t.a[n1 * R2 + k2].y = sn;
+      t.b[k2 * R1 + n1].x = c; t.b[k2 * R1 + n1].y = sn;
+    }
+  return t;
+}
+static __constant__ TwTab<128> c_tw128 = make_tw<128>();
+static __constant__ TwTab<96> c_tw96 = make_tw<96>();
+static __constant__ TwTab<48> c_tw48 = make_tw<48>();
+template <int N> __device__ __forceinline__ const TwTab<N> &tw_tab() {
+  if constexpr (N == 128) return c_tw128;
+  else if constexpr (N == 96) return c_tw96;
+  else { static_assert(N == 48, "no twiddle table for this length"); return c_tw48; }
+}
+
+// u[k] *= T[k] (S > 0) or conj T[k] (S < 0), k = 1..R-1
 template <int R, int S>
 __device__ __forceinline__ void twiddle_row(float2 (&u)[R], const float2 *T) {
-  static_assert(R % 2 == 0, "table rows hold an even number of factors");
-  const float4 *T4 = (const float4 *)T;
 #pragma unroll
-  for (int h = 0; h < R / 2; ++h) {
-    const float4 t = T4[h];
-    if (h > 0) u[2 * h] = S > 0 ? gkfft::cmul(u[2 * h], make_float2(t.x, t.y)) : gkfft::cmulc(u[2 * h], make_float2(t.x, t.y));
-    u[2 * h + 1] = S > 0 ? gkfft::cmul(u[2 * h + 1], make_float2(t.z, t.w)) : gkfft::cmulc(u[2 * h + 1], make_float2(t.z, t.w));
+  for (int k = 1; k < R; ++k) {
+    const float2 t = T[k];
+    u[k] = S > 0 ? gkfft::cmul(u[k], t) : gkfft::cmulc(u[k], t);
   }
 }
 
 // shared-memory bytes of the kernel below
 template <class ST, int MX_, int MY_, int NKY_, int NKX_>
 constexpr size_t ws2_smem_bytes() {
-  return (size_t)(2 * MX_ * (MY_ | 1) + 2 * MX_ + 2 * MY_) * 8 + (size_t)NKX_ * NKY_ * sizeof(ST) + 16 + 2 * GK_EB_N * 4;
+  return (size_t)(2 * MX_ * (MY_ | 1)) * 8 + (size_t)NKX_ * NKY_ * sizeof(ST) + 16 + 2 * GK_EB_N * 4;
 }
 
 // ---- lean epilogue role ------------------------------------------------------------------------
@@ -354,10 +377,6 @@ gk_stage_ws2_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkS
   float2 *sp = (float2 *)smem_raw;
   float2 *S = sp; sp += MX_ * LD;
   float2 *SG = sp; sp += MX_ * LD;
-  float2 *TX1 = sp; sp += MX_;   // [n1 < RX1][k2 < RX2] = wx^(n1 k2)
-  float2 *TXF = sp; sp += MX_;   // [k2 < RX2][n1 < RX1]
-  float2 *TY1 = sp; sp += MY_;   // [n1 < RY1][k2 < RY2] = wy^(n1 k2)
-  float2 *TYF = sp; sp += MY_;   // [k2 < RY2][n1 < RY1]
   ST *stg = (ST *)sp;            // the slab being transformed, landed by the bulk copy
   uint64_t *mbar = (uint64_t *)((unsigned char *)stg + slab * sizeof(ST));
   float *eblk = (float *)(mbar + 2);  // 16-byte aligned: slab-uniform epilogue coefficients, 2 slots
@@ -368,18 +387,6 @@ gk_stage_ws2_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkS
     // =============================== FFT role =====================================
     if constexpr (RF > 0) asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(RF));
     const gkfft::NamedSync<BAR_FFT, NTF> fsync;
-    for (int t = tid; t < MX_; t += NTF) {
-      const int n1 = t / RX2, k2 = t % RX2;
-      TX1[t] = P.twx[n1 * k2];
-      TXF[k2 * RX1 + n1] = P.twx[n1 * k2];
-    }
-    for (int t = tid; t < MY_; t += NTF) {
-      const int n1 = t / RY2, k2 = t % RY2;
-      TY1[t] = P.twy[n1 * k2];
-      TYF[k2 * RY1 + n1] = P.twy[n1 * k2];
-    }
-    fsync();
-
     // ---- X1: inverse x pass 1 of the spectral slab g (callable: slab index -> value) ----
     auto x1 = [&](auto g) {
       for (int w = tid; w < NC * RX1; w += NTF) {
@@ -411,7 +418,7 @@ gk_stage_ws2_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkS
           }
         });
         dft<RX2, +1>(u);
-        twiddle_row<RX2, +1>(u, TX1 + n1 * RX2);
+        twiddle_row<RX2, +1>(u, tw_tab<MX_>().a + n1 * RX2);
         float2 *q = S + n1 * LD + col;
 #pragma unroll
         for (int k2 = 0; k2 < RX2; ++k2) q[k2 * RX1 * LD] = u[k2];
@@ -419,26 +426,33 @@ gk_stage_ws2_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkS
     };
     // ---- X2: inverse x pass 2, in place ----
     auto x2 = [&]() {
-      for (int w = tid; w < NC * RX2; w += NTF) {
+      // two items per thread when the item count allows (same column, k2 and k2 + NTF/NC): both are loaded
+      // before either is transformed, so one shared-memory round trip covers both (the passes are
+      // latency-bound at 4 FFT warps per scheduler)
+      constexpr int ITEMS = NC * RX2, B = (ITEMS % (2 * NTF) == 0 && NTF % NC == 0) ? 2 : 1;
+      constexpr int BOFF = (NTF / NC) * RX1 * LD;
+      for (int w = tid; w < ITEMS; w += B * NTF) {
         const int c = w % NC, k2 = w / NC;
         if (c == NKY_) continue;
         const int col = c < NKY_ ? c : MY_ - (c - NKY_);
         float2 *q = S + k2 * RX1 * LD + col;
-        float2 u[RX1];
+        float2 u[B][RX1];
 #pragma unroll
-        for (int n1 = 0; n1 < RX1; ++n1) u[n1] = q[n1 * LD];
-        dft<RX1, +1>(u);
+        for (int b = 0; b < B; ++b)
 #pragma unroll
-        for (int k1 = 0; k1 < RX1; ++k1) q[k1 * LD] = u[k1];
+          for (int n1 = 0; n1 < RX1; ++n1) u[b][n1] = q[b * BOFF + n1 * LD];
+#pragma unroll
+        for (int b = 0; b < B; ++b) {
+          dft<RX1, +1>(u[b]);
+#pragma unroll
+          for (int k1 = 0; k1 < RX1; ++k1) q[b * BOFF + k1 * LD] = u[b][k1];
+        }
       }
     };
     // ---- Y1: inverse y pass 1, in place; the Hermitian-extended row is P(y) for 0 < y < nky,
     // conj of what sits at y > my - nky, Re P(0) at y = 0 (R15) and zero in between ----
     auto y1 = [&]() {
-      for (int w = tid; w < MX_ * RY1; w += NTF) {
-        const int r = w % MX_, n1 = w / MX_;
-        float2 *row = S + r * LD + n1;
-        float2 u[RY2];
+      auto load = [&](const float2 *row, int n1, float2 (&u)[RY2]) {
         sfor<0, RY2>([&](auto n2c) {
           constexpr int n2 = decltype(n2c)::value, off = RY1 * n2, hi = off + RY1 - 1;
           const int y = n1 + off;
@@ -458,10 +472,32 @@ gk_stage_ws2_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkS
           }
           u[n2] = v;
         });
+      };
+      // two items per thread when the item count allows (same row, n1 and n1 + NTF/mx): the second item's
+      // loads are issued between the first item's butterfly and its twiddle/store tail
+      constexpr int ITEMS = MX_ * RY1, B = (ITEMS % (2 * NTF) == 0 && NTF % MX_ == 0) ? 2 : 1;
+      constexpr int DN = NTF / MX_;
+      for (int w = tid; w < ITEMS; w += B * NTF) {
+        const int r = w % MX_, n1 = w / MX_;
+        float2 *row = S + r * LD + n1;
+        float2 u[RY2];
+        load(row, n1, u);
         dft<RY2, +1>(u);
-        twiddle_row<RY2, +1>(u, TY1 + n1 * RY2);
+        if constexpr (B == 2) {
+          float2 v[RY2];
+          load(row + DN, n1 + DN, v);
+          twiddle_row<RY2, +1>(u, tw_tab<MY_>().a + n1 * RY2);
 #pragma unroll
-        for (int k2 = 0; k2 < RY2; ++k2) row[k2 * RY1] = u[k2];
+          for (int k2 = 0; k2 < RY2; ++k2) row[k2 * RY1] = u[k2];
+          dft<RY2, +1>(v);
+          twiddle_row<RY2, +1>(v, tw_tab<MY_>().a + (n1 + DN) * RY2);
+#pragma unroll
+          for (int k2 = 0; k2 < RY2; ++k2) row[DN + k2 * RY1] = v[k2];
+        } else {
+          twiddle_row<RY2, +1>(u, tw_tab<MY_>().a + n1 * RY2);
+#pragma unroll
+          for (int k2 = 0; k2 < RY2; ++k2) row[k2 * RY1] = u[k2];
+        }
       }
     };
     // ---- Y2: inverse y pass 2, S -> dst (grad(chi) of the work item) ----
@@ -506,7 +542,7 @@ gk_stage_ws2_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkS
           u[k1] = make_float2(br[k1], g.y * u[k1].x - g.x * u[k1].y);
         }
         dft<RY1, -1>(u);
-        twiddle_row<RY1, -1>(u, TYF + k2 * RY1);
+        twiddle_row<RY1, -1>(u, tw_tab<MY_>().b + k2 * RY1);
 #pragma unroll
         for (int n1 = 0; n1 < RY1; ++n1) q0[n1] = u[n1];
       }
@@ -550,7 +586,7 @@ gk_stage_ws2_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkS
           u[k1] = hi ? make_float2(z.y + zc.y, zc.x - z.x) : make_float2(z.x + zc.x, z.y - zc.y);
         }
         dft<RX1, -1>(u);
-        twiddle_row<RX1, -1>(u, TXF + k2 * RX1);
+        twiddle_row<RX1, -1>(u, tw_tab<MX_>().b + k2 * RX1);
         float2 *d = S + k2 * RX1 * LD + NKY_ + m;
 #pragma unroll
         for (int n1 = 0; n1 < RX1; ++n1) d[n1 * LD] = u[n1];
