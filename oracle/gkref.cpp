@@ -591,6 +591,25 @@ void gkref_fluxes(const gkref *h, const double *f_in, const double *phi_in, doub
   }
 }
 
+// Spectra of the potential (ky_spec = sum_{s,kx} |phi|^2, kx_spec = sum_{s,ky} |phi|^2;
+// "the Parseval factor P_ky and parallel integration weight Delta s are applied"; R20:
+// both factors in both spectra, Delta s = 1/ns, P_m = 1 (m=0) or 2):
+//   kx_spec[p] = ds sum_i sum_m P_m |phi(i,p,m)|^2 ,   ky_spec[m] = ds P_m sum_i sum_p |phi(i,p,m)|^2
+void gkref_spectra(const gkref *h, const double *phi_in, double *kx_spec, double *ky_spec) {
+  const cplx *phi = (const cplx *)phi_in;
+  const double ds = 1.0 / h->ns;
+  for (int ip = 0; ip < h->nkx; ++ip) kx_spec[ip] = 0.0;
+  for (int m = 0; m < h->nky; ++m) ky_spec[m] = 0.0;
+  for (int i = 0; i < h->ns; ++i)
+    for (int ip = 0; ip < h->nkx; ++ip)
+      for (int m = 0; m < h->nky; ++m) {
+        const double P = (m == 0) ? 1.0 : 2.0;
+        const double a2 = std::norm(phi[h->pidx(i, ip, m)]);
+        kx_spec[ip] += ds * P * a2;
+        ky_spec[m] += ds * P * a2;
+      }
+}
+
 void gkref_bracket_slab(const gkref *h, const double *chi, const double *fs, int method, int mx,
                         int my, double *out) {
   h->bracket((const cplx *)chi, (const cplx *)fs, method, mx, my, (cplx *)out);

@@ -73,6 +73,9 @@ void gkref_rhs_slab(const gkref *, const double *f, const double *phi, int a, in
 void gkref_rk4_step(const gkref *, double *f, double dt);
 /* per-species (particle, heat, momentum) fluxes (R18): out[nspecies*3] */
 void gkref_fluxes(const gkref *, const double *f, const double *phi, double *out);
+/* kx and ky spectra of |phi|^2 with the Parseval factor and Delta s applied (R20):
+ * kx_spec[nkx], ky_spec[nky] */
+void gkref_spectra(const gkref *, const double *phi, double *kx_spec, double *ky_spec);
 
 /* bracket of two spectral slabs (nkx*nky complex each): 0.5*sum (k'x k''y - k'y k''x) chi f */
 void gkref_bracket_slab(const gkref *, const double *chi, const double *fs, int method, int mx,

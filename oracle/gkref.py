@@ -72,6 +72,7 @@ def _load():
         lib.gkref_rhs_slab.argtypes = [C.c_void_p, dp, dp, C.c_int, C.c_int, C.c_int, C.c_int, dp]
         lib.gkref_rk4_step.argtypes = [C.c_void_p, dp, C.c_double]
         lib.gkref_fluxes.argtypes = [C.c_void_p, dp, dp, dp]
+        lib.gkref_spectra.argtypes = [C.c_void_p, dp, dp, dp]
         lib.gkref_bracket_slab.argtypes = [C.c_void_p, dp, dp, C.c_int, C.c_int, C.c_int, dp]
         lib.gkref_table.restype = C.c_size_t
         lib.gkref_table.argtypes = [C.c_void_p, C.c_char_p, dp]
@@ -152,6 +153,13 @@ class GkRef:
         out = np.empty((self.nsp, 3), np.float64)
         _load().gkref_fluxes(self._h, _dp(f), _dp(phi), _dp(out))
         return out
+
+    def spectra(self, phi):
+        """(kx_spec[nkx], ky_spec[nky]) of |phi|^2 (PAPER.md:113, 390)."""
+        phi = self._c128(phi, self.phi_shape)
+        kxs, kys = np.empty(self.shape[4], np.float64), np.empty(self.shape[5], np.float64)
+        _load().gkref_spectra(self._h, _dp(phi), _dp(kxs), _dp(kys))
+        return kxs, kys
 
     def bracket_slab(self, chi, fs, method=0, mx=0, my=0):
         chi = self._c128(chi, self.shape[4:])
