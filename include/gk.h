@@ -101,6 +101,14 @@ int gk_rk4_steps(gk_ctx *ctx, void *f_dev, double dt, int nsteps);
  * parallel-momentum flux.  Synchronises the stream. */
 int gk_fluxes(gk_ctx *ctx, const void *f_dev, const void *phi_dev, double *out_host);
 
+/* Spectra of the potential (ky_spec = sum_{s,kx} |phi|^2, kx_spec = sum_{s,ky} |phi|^2, with the
+ * Parseval factor P_ky (1 at ky = 0, 2 otherwise) and the weight Delta s = 1/ns applied; R20):
+ *   kx_spec_host[p+K] = ds sum_{s,m} P_m |phi|^2   (nkx doubles),
+ *   ky_spec_host[m]   = ds P_m sum_{s,p} |phi|^2   (nky doubles).
+ * phi_dev: device, [ns][nkx][nky] complex64 (as written by gk_field_solve).  Accumulates in double,
+ * deterministic (one block tree per output, no atomics).  Synchronises the stream.  GK_EINVAL on null. */
+int gk_spectra(gk_ctx *ctx, const void *phi_dev, double *kx_spec_host, double *ky_spec_host);
+
 /* Test hook: copies a create-time table to host memory as doubles.  `which` is one of
  * "vpar","mu","wmu","kx","ky","B","F","BG","J0","Gamma0","FM","den","zonal","pad".  Returns the
  * number of doubles (also when host_out is NULL), 0 for an unknown name. */

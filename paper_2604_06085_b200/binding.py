@@ -84,6 +84,7 @@ def load_library(build_if_missing: bool = True):
     lib.gk_rk4_step.argtypes = [vp, vp, C.c_double]
     lib.gk_rk4_steps.argtypes = [vp, vp, C.c_double, C.c_int]
     lib.gk_fluxes.argtypes = [vp, vp, vp, dp]
+    lib.gk_spectra.argtypes = [vp, vp, dp, dp]
     lib.gk_export_table.restype = C.c_size_t
     lib.gk_export_table.argtypes = [vp, C.c_char_p, dp, C.c_size_t]
     lib.gk_launch_count.restype = C.c_longlong
@@ -225,6 +226,15 @@ class GkContext:
         self._check(self.lib.gk_fluxes(self._h, C.c_void_p(f.data_ptr()), C.c_void_p(phi.data_ptr()),
                                        out.ctypes.data_as(C.POINTER(C.c_double))))
         return out
+
+    def gk_spectra(self, phi):
+        """(kx_spec[nkx], ky_spec[nky]) of |phi|^2 (PAPER.md:113, 390)."""
+        import numpy as np
+        kxs, kys = np.zeros(self.shape[4], np.float64), np.zeros(self.shape[5], np.float64)
+        self._check(self.lib.gk_spectra(self._h, C.c_void_p(phi.data_ptr()),
+                                        kxs.ctypes.data_as(C.POINTER(C.c_double)),
+                                        kys.ctypes.data_as(C.POINTER(C.c_double))))
+        return kxs, kys
 
     def gk_export_table(self, which: str):
         import numpy as np

@@ -23,6 +23,12 @@ UNITS = [
 ]
 DEPS = ["gk_lib.cu", "gk_stage_inst.cu", "gk_kernels.cuh", "gk_common.cuh", "gk_stage.cuh", "gk_stage_ws.cuh", "gk_stage_ws2.cuh", "gk_fft.cuh", "gk_tables.h",
         "gk_dev.h", "gk_pick.h"]
+# per translation unit: a unit is recompiled only if its object is older than one of these
+UNIT_DEPS = {
+    "gk_lib.cu": ["gk_lib.cu", "gk_kernels.cuh", "gk_common.cuh", "gk_fft.cuh", "gk_tables.h", "gk_dev.h", "gk_pick.h"],
+    "gk_stage_inst.cu": ["gk_stage_inst.cu", "gk_common.cuh", "gk_stage.cuh", "gk_stage_ws.cuh", "gk_stage_ws2.cuh",
+                         "gk_fft.cuh", "gk_dev.h", "gk_pick.h"],
+}
 
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
@@ -55,9 +61,17 @@ def build(force: bool = False, verbose: bool = False) -> str:
     units = UNITS[:2] if fast else UNITS
     extra = ["-DGK_ONLY_C64"] if fast else []
 
+    flagfile = os.path.join(OBJDIR, "flags.txt")
+    flags_now = " ".join([*NVCC_FLAGS, *extra])
+    same_flags = os.path.exists(flagfile) and open(flagfile).read() == flags_now
+
     def compile_unit(u):
         src, defs, obj = u
-        cmd = [_nvcc(), *NVCC_FLAGS, *extra, *defs, "-c", os.path.join(CSRC, src), "-o", os.path.join(OBJDIR, obj)]
+        objp = os.path.join(OBJDIR, obj)
+        cmd = [_nvcc(), *NVCC_FLAGS, *extra, *defs, "-c", os.path.join(CSRC, src), "-o", objp]
+        deps = [os.path.join(CSRC, d) for d in UNIT_DEPS[src]] + [os.path.join(INCLUDE, "gk.h")]
+        if not force and same_flags and os.path.exists(objp) and all(os.path.getmtime(d) <= os.path.getmtime(objp) for d in deps):
+            return cmd, subprocess.CompletedProcess(cmd, 0, "(up to date)\n", "")
         res = subprocess.run(cmd, capture_output=True, text=True)
         return cmd, res
 
@@ -80,6 +94,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
         sys.stderr.write(log)
         raise RuntimeError("nvcc failed building libgk.so")
     os.replace(tmp, LIB)
+    with open(flagfile, "w") as fh:
+        fh.write(flags_now)
     if verbose:
         print(log)
     return LIB

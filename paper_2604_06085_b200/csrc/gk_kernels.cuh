@@ -119,5 +119,30 @@ __global__ void __launch_bounds__(256) gk_flux_kernel(const __grid_constant__ Gk
   }
 }
 
-}  // namespace gk
+// Spectra of |phi|^2 (R20).  Block b < nkx sums row p = b over (s, ky) with the Parseval
+// factor; block nkx + m sums column m over (s, kx).  One deterministic tree per output, double accumulation.
+__global__ void __launch_bounds__(256) gk_spectra_kernel(const __grid_constant__ GkDev P,
+                                                         const float2 *__restrict__ phi, double *out) {
+  const int b = blockIdx.x;
+  const bool row = b < P.nkx;
+  const int fixed = row ? b : b - P.nkx;        // p (row) or m (column)
+  const int nfree = row ? P.nky : P.nkx;
+  double acc = 0.0;
+  for (int q = threadIdx.x; q < P.ns * nfree; q += 256) {
+    const int i = q / nfree, r = q - i * nfree;
+    const int p = row ? fixed : r, m = row ? r : fixed;
+    const float2 v = phi[(long long)i * P.slab + p * P.nky + m];
+    const double a2 = (double)v.x * v.x + (double)v.y * v.y;
+    acc += (m == 0 ? 1.0 : 2.0) * a2;
+  }
+  __shared__ double red[256];
+  red[threadIdx.x] = acc;
+  __syncthreads();
+  for (int h = 128; h > 0; h >>= 1) {
+    if (threadIdx.x < h) red[threadIdx.x] += red[threadIdx.x + h];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) out[b] = red[0] / P.ns;
+}
 
+}  // namespace gk

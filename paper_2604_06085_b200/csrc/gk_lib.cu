@@ -478,6 +478,24 @@ int gk_fluxes(gk_ctx *c, const void *f, const void *phi, double *out_host) {
   return GK_OK;
 }
 
+int gk_spectra(gk_ctx *c, const void *phi, double *kx_spec, double *ky_spec) {
+  if (int r = usable(c)) return r;
+  if (!phi || !kx_spec || !ky_spec) return fail(c, GK_EINVAL, "gk_spectra: null pointer");
+  const int n = c->P.nkx + c->P.nky;
+  double *d = nullptr;
+  GK_CUDA(c, cudaMalloc(&d, n * sizeof(double)));
+  gk::gk_spectra_kernel<<<n, 256, 0, c->stream>>>(c->P, (const float2 *)phi, d);
+  ++c->launches;
+  std::vector<double> h(n);
+  cudaError_t e = cudaMemcpyAsync(h.data(), d, n * sizeof(double), cudaMemcpyDeviceToHost, c->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+  cudaFree(d);
+  if (e != cudaSuccess) return fail(c, GK_ECUDA, std::string("gk_spectra: ") + cudaGetErrorString(e));
+  std::memcpy(kx_spec, h.data(), c->P.nkx * sizeof(double));
+  std::memcpy(ky_spec, h.data() + c->P.nkx, c->P.nky * sizeof(double));
+  return GK_OK;
+}
+
 size_t gk_export_table(const gk_ctx *c, const char *which, double *out, size_t maxn) {
   if (!c || !which) return 0;
   const gkt::Tables &T = c->T;

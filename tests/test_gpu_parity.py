@@ -151,6 +151,19 @@ def test_half_storage_variant(storage):
     assert rel_l2(g.from_state(fd), o.rk4_step(fq, cfg["dt"], n)) < TOL_HALF
 
 
+def test_spectra_parity():
+    # PAPER.md:113, 390; R20.  Both sides sum the same fp32 phi in double: agreement to rounding order.
+    cfg = small_cfg(**MID)
+    g, o = _ctx(cfg), GkRef(cfg)
+    f = rand_c(np.random.default_rng(41), o.shape, True).astype(np.complex64)
+    phi = g.gk_field_solve(g.to_state(f))
+    kxs, kys = g.gk_spectra(phi)
+    rx, ry = o.spectra(phi.cpu().numpy())
+    np.testing.assert_allclose(kxs, rx, rtol=1e-12)
+    np.testing.assert_allclose(kys, ry, rtol=1e-12)
+    assert abs(kxs.sum() - kys.sum()) < 1e-12 * kxs.sum()
+
+
 def test_fluxes_parity_and_particle_flux_invariant():
     cfg = small_cfg(**MID)
     g, o = _ctx(cfg), GkRef(cfg)
