@@ -97,6 +97,14 @@ int gk_rhs(gk_ctx *ctx, const void *f_dev, void *phi_dev, void *rhs_dev);
 int gk_rk4_step(gk_ctx *ctx, void *f_dev, double dt);
 int gk_rk4_steps(gk_ctx *ctx, void *f_dev, double dt, int nsteps);
 
+/* One RK4 step with HOST buffers (bench.py's end-to-end leg): copies f_host_in -> f_dev, runs gk_rk4_step on
+ * f_dev, copies f_dev -> f_host_out, all asynchronous on the context stream in that order (truly asynchronous
+ * only for pinned host memory; pageable memory makes the copies synchronous).  f_host_in / f_host_out: host,
+ * same layout and storage type as f, may alias; f_dev: device scratch of the size of f, caller-owned.  Does
+ * not synchronise at the end: synchronise the stream before reading f_host_out.  GK_EINVAL on null pointers
+ * or a workspace too small for gk_rk4_step. */
+int gk_rk4_step_host(gk_ctx *ctx, const void *f_host_in, void *f_host_out, void *f_dev, double dt);
+
 /* Transport fluxes per species (R18): out_host[3*a + {0,1,2}] = particle, heat,
  * parallel-momentum flux.  Synchronises the stream. */
 int gk_fluxes(gk_ctx *ctx, const void *f_dev, const void *phi_dev, double *out_host);

@@ -84,6 +84,7 @@ def load_library(build_if_missing: bool = True):
     lib.gk_rk4_step.argtypes = [vp, vp, C.c_double]
     lib.gk_rk4_steps.argtypes = [vp, vp, C.c_double, C.c_int]
     lib.gk_fluxes.argtypes = [vp, vp, vp, dp]
+    lib.gk_rk4_step_host.argtypes = [vp, vp, vp, vp, C.c_double]
     lib.gk_spectra.argtypes = [vp, vp, dp, dp]
     lib.gk_export_table.restype = C.c_size_t
     lib.gk_export_table.argtypes = [vp, C.c_char_p, dp, C.c_size_t]
@@ -218,6 +219,16 @@ class GkContext:
         self._chk_state(f, "f")
         self._check(self.lib.gk_rk4_steps(self._h, C.c_void_p(f.data_ptr()), C.c_double(dt), int(nsteps)))
         return f
+
+    def gk_rk4_step_host(self, f_host_in, f_host_out, f_dev, dt: float):
+        """One RK4 step on host buffers (torch CPU tensors, pinned for asynchronous copies) through the
+        device scratch f_dev; asynchronous on the context stream."""
+        self._chk_state(f_dev, "f_dev")
+        for t in (f_host_in, f_host_out):
+            if t.device.type != "cpu" or not t.is_contiguous() or t.numel() != f_dev.numel() or t.dtype != f_dev.dtype:
+                raise ValueError("host buffers must be contiguous CPU tensors of the shape and dtype of f")
+        self._check(self.lib.gk_rk4_step_host(self._h, C.c_void_p(f_host_in.data_ptr()), C.c_void_p(f_host_out.data_ptr()),
+                                              C.c_void_p(f_dev.data_ptr()), float(dt)))
 
     def gk_fluxes(self, f, phi):
         import numpy as np

@@ -455,6 +455,16 @@ int gk_rk4_steps(gk_ctx *c, void *f, double dt, int nsteps) {
 
 int gk_rk4_step(gk_ctx *c, void *f, double dt) { return gk_rk4_steps(c, f, dt, 1); }
 
+int gk_rk4_step_host(gk_ctx *c, const void *f_host_in, void *f_host_out, void *f_dev, double dt) {
+  if (int r = usable(c)) return r;
+  if (!f_host_in || !f_host_out || !f_dev) return fail(c, GK_EINVAL, "gk_rk4_step_host: null pointer");
+  const size_t bytes = (size_t)c->P.ntot * c->elem_bytes;
+  GK_CUDA(c, cudaMemcpyAsync(f_dev, f_host_in, bytes, cudaMemcpyHostToDevice, c->stream));
+  if (int r = gk_rk4_steps(c, f_dev, dt, 1)) return r;
+  GK_CUDA(c, cudaMemcpyAsync(f_host_out, f_dev, bytes, cudaMemcpyDeviceToHost, c->stream));
+  return GK_OK;
+}
+
 int gk_fluxes(gk_ctx *c, const void *f, const void *phi, double *out_host) {
   if (int r = usable(c)) return r;
   if (!f || !phi || !out_host) return fail(c, GK_EINVAL, "gk_fluxes: null pointer");

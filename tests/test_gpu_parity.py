@@ -151,6 +151,22 @@ def test_half_storage_variant(storage):
     assert rel_l2(g.from_state(fd), o.rk4_step(fq, cfg["dt"], n)) < TOL_HALF
 
 
+def test_rk4_step_host_buffers_equal_the_device_call():
+    # gk_rk4_step_host = H2D + gk_rk4_step + D2H on the context stream: bit-identical to the device call
+    import torch
+    cfg = small_cfg(**MID)
+    g = _ctx(cfg)
+    f = rand_c(np.random.default_rng(43), gkinputs.f_shape(cfg), True).astype(np.complex64) * 1e-3
+    fd = g.to_state(f)
+    hin = fd.cpu().pin_memory()
+    hout = torch.empty_like(hin).pin_memory()
+    scratch = g.empty_state()
+    g.gk_rk4_step_host(hin, hout, scratch, cfg["dt"])
+    g.gk_rk4_step(fd, cfg["dt"])
+    torch.cuda.synchronize()
+    assert torch.equal(hout, fd.cpu())
+
+
 def test_spectra_parity():
     # PAPER.md:113, 390; R20.  Both sides sum the same fp32 phi in double: agreement to rounding order.
     cfg = small_cfg(**MID)
