@@ -37,7 +37,8 @@ struct gk_ctx {
   bool poisoned = false;
   int num_sms = 0;
   int stage_grid = 0;
-  int stage_threads = 512, stage_occ = 1, stage_ws = 0, stage_kind = 0;
+  int stage_threads = 512, stage_occ = 1, stage_ws = 0, stage_kind = 0, host_moment = 0;
+  size_t stage_gchi = 0;
   size_t stage_smem = 0;
   size_t elem_bytes = 8;
   // workspace
@@ -268,6 +269,8 @@ int gk_create(const gk_grid *g, const gk_species *sp, const gk_salpha *geo, cons
     c->stage_occ = pick.occ;
     c->stage_ws = pick.ws;
     c->stage_kind = pick.kind;
+    c->host_moment = pick.host_moment;
+    c->stage_gchi = pick.gchi;
     const int resident = c->num_sms * pick.occ;  // persistent CTAs
 
     // work decomposition: items (a, l, vpar chunk, i) are dealt round-robin to the persistent CTAs.
@@ -357,7 +360,8 @@ int gk_create(const gk_grid *g, const gk_species *sp, const gk_salpha *geo, cons
   c->off_mom = off; off += align256((size_t)P.nparts * P.nphi * 8);
   c->off_phi = off; off += align256((size_t)P.nphi * 8);
   c->off_gchi = off;
-  if (nl && !P.gchi_in_smem) off += align256((size_t)c->stage_grid * P.mx * P.ldy * 8);
+  if (nl && c->stage_gchi) off += align256((size_t)c->stage_grid * c->stage_gchi * 8);
+  else if (nl && !P.gchi_in_smem) off += align256((size_t)c->stage_grid * P.mx * P.ldy * 8);
   c->off_chis = off; off += align256((size_t)c->stage_grid * (c->stage_ws ? 9 : 3) * P.slab * 8);
   c->off_nl = off;
   if (c->stage_ws) off += align256((size_t)c->stage_grid * 2 * P.slab * 8);
@@ -437,17 +441,28 @@ int gk_rk4_steps(gk_ctx *c, void *f, double dt, int nsteps) {
     }
     // classical RK4: acc = f + dt/6 k1, then += dt/3 k2, += dt/3 k3, f = acc + dt/6 k4
     if (int r = solve_phi_from_planes(c, mom, phi)) return r;
+    // kernels that do not accumulate the moment of the new state themselves are followed by gk_moment_kernel
+    auto moment_of = [&](const void *state) {
+      if (!c->host_moment) return;
+#define GK_CALL(ST) launch_moment<ST>(c, state, mom)
+      GK_BY_STORAGE(c, GK_CALL);
+#undef GK_CALL
+    };
     A.mode = 1; A.y = f; A.fn = f; A.out = ya; A.c = 0.5f * h; A.b = h / 6.f;
     stage_launch(c, A);
+    moment_of(ya);
     if (int r = solve_phi_from_planes(c, mom, phi)) return r;
     A.mode = 2; A.y = ya; A.fn = f; A.out = yb; A.c = 0.5f * h; A.b = h / 3.f;
     stage_launch(c, A);
+    moment_of(yb);
     if (int r = solve_phi_from_planes(c, mom, phi)) return r;
     A.mode = 2; A.y = yb; A.fn = f; A.out = ya; A.c = h; A.b = h / 3.f;
     stage_launch(c, A);
+    moment_of(ya);
     if (int r = solve_phi_from_planes(c, mom, phi)) return r;
     A.mode = 3; A.y = ya; A.fn = f; A.out = f; A.c = 0.f; A.b = h / 6.f;
     stage_launch(c, A);
+    moment_of(f);
     if (int r = check_launch(c, "stage kernel")) return r;
   }
   return GK_OK;

@@ -6,7 +6,9 @@
 // ws: FFT-role threads of the warp-specialised kernels (0: unified kernel); smem > 0: the kernel's own
 // fixed shared-memory plan (gk_stage_ws2_kernel), 0: planned by gk_create
 // kind: 0 gk_stage_kernel, 1 gk_stage_ws_kernel, 2 gk_stage_ws2_kernel, 3 gk_stage_lin_kernel
-struct StagePick { const void *fn; int threads; int occ; int ws; size_t smem; int kind; };
+// 4 gk_stage_ws3_kernel.  gchi: elements of per-CTA grad(chi) scratch the kernel needs regardless of the
+// shared-memory plan; host_moment: the kernel does not write the moment planes (gk_moment_kernel follows it)
+struct StagePick { const void *fn; int threads; int occ; int ws; size_t smem; int kind; size_t gchi; int host_moment; };
 
 // storage 0: complex64, 1: complex fp16, 2: complex bf16
 StagePick gk_pick_stage_c64(int mx, int my, int nky, int nkx, bool nl, int force_occ, int force_thr, int ws_ntf);
@@ -15,7 +17,7 @@ StagePick gk_pick_stage_bf16(int mx, int my, int nky, int nkx, bool nl, int forc
 
 inline StagePick gk_pick_stage(int storage, int mx, int my, int nky, int nkx, bool nl, int force_occ, int force_thr, int ws_ntf) {
 #ifdef GK_ONLY_C64
-  if (storage != 0) return {nullptr, 0, 0, 0, 0, 0};
+  if (storage != 0) return {nullptr, 0, 0, 0, 0, 0, 0, 0};
 #else
   if (storage == 1) return gk_pick_stage_f16(mx, my, nky, nkx, nl, force_occ, force_thr, ws_ntf);
   if (storage == 2) return gk_pick_stage_bf16(mx, my, nky, nkx, nl, force_occ, force_thr, ws_ntf);

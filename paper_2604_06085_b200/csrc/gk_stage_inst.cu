@@ -4,6 +4,7 @@
 #include "gk_stage.cuh"
 #include "gk_stage_ws.cuh"
 #include "gk_stage_ws2.cuh"
+#include "gk_stage_ws3.cuh"
 #include "gk_pick.h"
 
 #ifndef GK_ST_ID
@@ -46,7 +47,7 @@ template <class ST> StagePick pick_stage(int mx, int my, int nky, int nkx, bool 
   GK_SPEC_LIN(32, 85);
   GK_SPEC_LIN(64, 127);
 #undef GK_SPEC_LIN
-  return {nullptr, 0, 0, 0, 0, 0};
+  return {nullptr, 0, 0, 0, 0, 0, 0, 0};
 }
 // preference order of (threads, occ) variants; the first one that exists and fits is used
 // warp-specialised variants (FFT-role threads, epilogue-role threads)
@@ -59,7 +60,7 @@ template <class ST> StagePick pick_stage_ws(int mx, int my, int nky, int nkx, in
   GK_WS(128, 96, 32, 85, 768, 256);
   GK_WS(192, 192, 64, 127, 512, 512);
 #undef GK_WS
-  return {nullptr, 0, 0, 0, 0, 0};
+  return {nullptr, 0, 0, 0, 0, 0, 0, 0};
 }
 // in-place variants (gk_stage_ws2_kernel): the padded field and grad(chi) both live in shared memory.
 // `code` = FFT-role threads, +1, +2, ... for the alternative role splits (GK_WS_NTF, tuning).
@@ -75,7 +76,7 @@ template <class ST> StagePick pick_stage_ws2(int mx, int my, int nky, int nkx, i
   GK_WS2(512, 128, 48, 16, 85, 512, 384, 56, 88, 1);
   GK_WS2(513, 128, 48, 16, 85, 512, 256, 56, 128, 2);
 #undef GK_WS2
-  return {nullptr, 0, 0, 0, 0, 0};
+  return {nullptr, 0, 0, 0, 0, 0, 0, 0};
 }
 // term III off: lean streaming kernel (gk_stage_lin_kernel); `code` selects (threads, points in flight, CTAs per SM)
 template <class ST> StagePick pick_stage_lin(int nky, int nkx, int code) {
@@ -87,13 +88,25 @@ template <class ST> StagePick pick_stage_lin(int nky, int nkx, int code) {
   GK_LIN(0, 16, 85, 512, 2, 1);
   GK_LIN(0, 64, 127, 512, 2, 1);
 #undef GK_LIN
-  return {nullptr, 0, 0, 0, 0, 0};
+  return {nullptr, 0, 0, 0, 0, 0, 0, 0};
+}
+// row-streaming variant (gk_stage_ws3_kernel): padded grids whose real-space field does not fit shared memory
+template <class ST> StagePick pick_stage_ws3(int mx, int my, int nky, int nkx, int code) {
+#define GK_WS3(CODE, MX, MY, NKY, NKX, RC, NTF, NTE)                              \
+  if (mx == MX && my == MY && nky == NKY && nkx == NKX && code == CODE)           \
+    return {(const void *)gk::gk_stage_ws3_kernel<ST, MX, MY, NKY, NKX, RC, NTF, NTE>, NTF + NTE, 1, NTF, \
+            gk::ws3_smem_bytes<ST, MX, MY, NKY, NKX, RC>(), 4, (size_t)MX * MY, 1}
+  GK_WS3(512, 192, 192, 64, 127, 24, 512, 512);
+#undef GK_WS3
+  return {nullptr, 0, 0, 0, 0, 0, 0, 0};
 }
 template <class ST> StagePick pick_stage_auto(int mx, int my, int nky, int nkx, bool nl, int force_occ, int force_thr, int ws_ntf) {
   const bool ws_old = ws_ntf < 0;  // negative: the chunked warp-specialised kernel (gk_stage_ws_kernel)
   if (ws_old) ws_ntf = -ws_ntf;
   if (nl && ws_ntf > 0) {
-    StagePick p = ws_old ? StagePick{nullptr, 0, 0, 0, 0, 0} : pick_stage_ws2<ST>(mx, my, nky, nkx, ws_ntf);
+    StagePick p = ws_old ? StagePick{nullptr, 0, 0, 0, 0, 0, 0, 0} : pick_stage_ws2<ST>(mx, my, nky, nkx, ws_ntf);
+    if (p.fn) return p;
+    if (!ws_old) p = pick_stage_ws3<ST>(mx, my, nky, nkx, ws_ntf);
     if (p.fn) return p;
     p = pick_stage_ws<ST>(mx, my, nky, nkx, ws_ntf);
     if (p.fn) return p;

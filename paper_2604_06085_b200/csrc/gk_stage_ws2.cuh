@@ -79,8 +79,10 @@ template <int N> constexpr TwTab<N> make_tw() {
 static __constant__ TwTab<128> c_tw128 = make_tw<128>();
 static __constant__ TwTab<96> c_tw96 = make_tw<96>();
 static __constant__ TwTab<48> c_tw48 = make_tw<48>();
+static __constant__ TwTab<192> c_tw192 = make_tw<192>();
 template <int N> __device__ __forceinline__ const TwTab<N> &tw_tab() {
   if constexpr (N == 128) return c_tw128;
+  else if constexpr (N == 192) return c_tw192;
   else if constexpr (N == 96) return c_tw96;
   else { static_assert(N == 48, "no twiddle table for this length"); return c_tw48; }
 }
@@ -108,7 +110,10 @@ constexpr size_t ws2_smem_bytes() {
 // the kx connection folded into one per-thread offset (R6) and one predicate per point
 // (open chain end: PAPER.md:350, 362; R7).
 
-template <class ST, int NKY_, int NKX_, int NTF, int NTE, int NB>
+// MACC: the velocity-space moment of the new state is accumulated in registers over the vpar march (one
+// float2 per point of the thread); false for slabs too large for that (the host then runs gk_moment_kernel
+// on the new state).
+template <class ST, int NKY_, int NKX_, int NTF, int NTE, int NB, bool MACC = true>
 __device__ __forceinline__ void ws_epilogue_role2(const GkDev &P, const GkStageArgs &A, float2 *chis_cta,
                                                   const float2 *nl_cta, float *eblk, int tid) {
   constexpr int NT = NTF + NTE;
@@ -156,9 +161,9 @@ __device__ __forceinline__ void ws_epilogue_role2(const GkDev &P, const GkStageA
       else if (i2 < 0) { i2 += P.ns; wrap = -1; }
       soff[q] = (i2 - i) * slab + wrap * mk * nky;
     }
-    float2 macc[EPT];
+    float2 macc[MACC ? EPT : 1];
 #pragma unroll
-    for (int k = 0; k < EPT; ++k) macc[k] = make_float2(0.f, 0.f);
+    for (int k = 0; k < (MACC ? EPT : 1); ++k) macc[k] = make_float2(0.f, 0.f);
     const int j0 = c * P.jchunk, j1 = min(P.nv, (c + 1) * P.jchunk);
     for (int j = j0; j < j1; ++j, ++u) {
       // coefficient block: one per CTA and slab parity beside an FFT role (published by BAR_FULL), one per warp otherwise
@@ -315,7 +320,7 @@ __device__ __forceinline__ void ws_epilogue_role2(const GkDev &P, const GkStageA
                 out = gkfft::caxpy(A.b, r, ac[q]);
               }
               Cv<ST>::stcs(outp, eo, out);
-              macc[k] = cadd(macc[k], out);
+              if constexpr (MACC) macc[k] = cadd(macc[k], out);
             }
           }
           asm volatile("" ::: "memory");      // the next batch's loads stay below this one's arithmetic
@@ -333,13 +338,13 @@ __device__ __forceinline__ void ws_epilogue_role2(const GkDev &P, const GkStageA
       }
       if constexpr (NL) bar_arrive_n(BAR_FREE + (u & 1), NT);
     }
-    if (A.mom) {
+    if (MACC && A.mom) {
       // moment plane of this item: Z n 2 pi w_v B_i w_mu J0 sum_j f   (a1 of the next stage)
       const float momw = P.sp[a].momfac * P.wmu[l] * P.B[i];
       const float *j0p = P.J0 + (((long long)a * P.nmu + l) * P.ns + i) * P.slab;
       float2 *dst = A.mom + (((long long)a * P.nmu + l) * P.nchunk + c) * P.nphi + (long long)i * P.slab;
 #pragma unroll
-      for (int k = 0; k < EPT; ++k) {
+      for (int k = 0; k < (MACC ? EPT : 1); ++k) {
         const int e = et + k * NTE;
         if (e < slab) dst[e] = gkfft::cscale(momw * __ldg(&j0p[e]), macc[k]);
       }
