@@ -9,7 +9,7 @@
 //   grad(chi)            per-CTA scratch in L2, stored in the order the fused pass reads it:
 //                        [chunk][k2][k1][row of the chunk] -> lanes read consecutive addresses
 // per slab: X1, X2, then per chunk Y1 (XA -> W), YF (inverse y pass 2 + bracket + forward y pass 1,
-// in registers), F2, UN (two-for-one unpack into XA); XF1, XF2 -> bracket ring for the epilogue
+// in registers), F2U (forward y pass 2 + two-for-one unpack into XA, partners exchanged by shuffles); XF1, XF2 -> bracket ring for the epilogue
 // role (ws_epilogue_role2 without register moments: gk_moment_kernel runs on the new state).
 #pragma once
 
@@ -178,36 +178,38 @@ gk_stage_ws3_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkS
         for (int n1 = 0; n1 < RY1; ++n1) q0[n1] = u[n1];
       }
     };
-    // ---- F2: forward y pass 2 of the packed rows, in place; only the retained ky and their mirrors ----
-    auto f2 = [&]() {
-      for (int w = tid; w < HC * RY1; w += NTF) {
-        const int p = w % HC, n1 = w / HC;
-        float2 *row = W + p * LDW + n1;
+    // ---- F2U: forward y pass 2 of the packed rows fused with the two-for-one unpack.  A warp holds PW pairs x
+    // RY1 residues n1; the thread (p, n1) ends with Z(n1 + RY1 n2) and needs Z(my - y) for its retained
+    // y = n1 + RY1 n2 < nky, which is output RY2-1-n2 of the thread (p, RY1 - n1) (its own output RY2 - n2
+    // when n1 = 0): one shuffle per retained value.  Row r0+p of XA gets A(m) = Z(m) + conj Z(my-m), row
+    // r0+p+HC gets B(m) = -i (Z(m) - conj Z(my-m)) (factor 1/2 in the epilogue's scale). ----
+    auto f2u = [&](int r0) {
+      constexpr int PW = 32 / RY1, NLOW = (NKY_ + RY1 - 1) / RY1;
+      static_assert(PW >= 1 && HC % PW == 0 && NLOW < RY2, "pairs per warp");
+      const int lane = tid & 31, wq = lane / RY1, n1 = lane - wq * RY1;
+      const bool active = lane < PW * RY1;
+      const int n1p = (n1 == 0) ? 0 : RY1 - n1;
+      const int src = active ? wq * RY1 + n1p : lane;
+      for (int wp = tid >> 5; wp < HC / PW; wp += NTF / 32) {
+        const int p = wp * PW + (active ? wq : 0);
+        const float2 *row = W + p * LDW + n1;
         float2 u[RY2];
 #pragma unroll
-        for (int k2 = 0; k2 < RY2; ++k2) u[k2] = row[k2 * RY1];
+        for (int k2 = 0; k2 < RY2; ++k2) u[k2] = active ? row[k2 * RY1] : make_float2(0.f, 0.f);
         dft<RY2, -1>(u);
-        sfor<0, RY2>([&](auto n2c) {
-          constexpr int n2 = decltype(n2c)::value, off = RY1 * n2, hi = off + RY1 - 1;
-          if constexpr (off >= NKY_ && hi <= MY_ - NKY_) {
-          } else if constexpr (hi < NKY_ || off > MY_ - NKY_) {
-            row[off] = u[n2];
-          } else {
-            const int y = n1 + off;
-            if (y < NKY_ || y > MY_ - NKY_) row[off] = u[n2];
+        float2 *da = XA + (r0 + p) * LDX + n1, *db = da + HC * LDX;
+        sfor<0, NLOW>([&](auto n2c) {
+          constexpr int n2 = decltype(n2c)::value;
+          const float2 mine = (n1 == 0) ? u[n2 == 0 ? 0 : RY2 - n2] : u[RY2 - 1 - n2];   // what my partner needs
+          float2 zc;
+          zc.x = __shfl_sync(0xffffffffu, mine.x, src);
+          zc.y = __shfl_sync(0xffffffffu, mine.y, src);
+          const float2 z = u[n2];
+          if (active && n1 + RY1 * n2 < NKY_) {
+            da[RY1 * n2] = make_float2(z.x + zc.x, z.y - zc.y);
+            db[RY1 * n2] = make_float2(z.y + zc.y, zc.x - z.x);
           }
         });
-      }
-    };
-    // ---- UN: two-for-one unpack of the chunk into XA's P columns: row r0+p gets A(m) = Z(m) + conj Z(my-m),
-    // row r0+p+HC gets B(m) = -i (Z(m) - conj Z(my-m)) (factor 1/2 in the epilogue's scale) ----
-    auto un = [&](int r0) {
-      for (int w = tid; w < HC * NKY_; w += NTF) {
-        const int m = w % NKY_, p = w / NKY_;
-        const float2 z = W[p * LDW + m];
-        const float2 zc = W[p * LDW + (m == 0 ? 0 : MY_ - m)];
-        XA[(r0 + p) * LDX + m] = make_float2(z.x + zc.x, z.y - zc.y);
-        XA[(r0 + p + HC) * LDX + m] = make_float2(z.y + zc.y, zc.x - z.x);
       }
     };
     // ---- XF1: forward x pass 1 of the nky retained columns, in place ----
@@ -282,9 +284,7 @@ gk_stage_ws3_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkS
           fsync();
           yf(ch);
           fsync();
-          f2();
-          fsync();
-          un(ch * RC_);
+          f2u(ch * RC_);
           fsync();
         }
         xf1();
