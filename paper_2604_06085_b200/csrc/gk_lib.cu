@@ -360,9 +360,14 @@ int gk_create(const gk_grid *g, const gk_species *sp, const gk_salpha *geo, cons
   c->off_mom = off; off += align256((size_t)P.nparts * P.nphi * 8);
   c->off_phi = off; off += align256((size_t)P.nphi * 8);
   c->off_gchi = off;
-  if (nl && c->stage_gchi) off += align256((size_t)c->stage_grid * c->stage_gchi * 8);
+  // gk_stage_ws3_kernel (kind 4): scratch per (species, mu, s), shared by the CTAs that work on its vpar chunks
+  const size_t n_li = (size_t)T.nsp * T.nmu * T.ns;
+  if (nl && c->stage_kind == 4) off += align256(n_li * c->stage_gchi * 8);
+  else if (nl && c->stage_gchi) off += align256((size_t)c->stage_grid * c->stage_gchi * 8);
   else if (nl && !P.gchi_in_smem) off += align256((size_t)c->stage_grid * P.mx * P.ldy * 8);
-  c->off_chis = off; off += align256((size_t)c->stage_grid * (c->stage_ws ? 9 : 3) * P.slab * 8);
+  c->off_chis = off;
+  if (c->stage_kind == 4) off += align256(n_li * 3 * P.slab * 8);
+  else off += align256((size_t)c->stage_grid * (c->stage_ws ? 9 : 3) * P.slab * 8);
   c->off_nl = off;
   if (c->stage_ws) off += align256((size_t)c->stage_grid * 2 * P.slab * 8);
   c->need_rhs = off;

@@ -113,7 +113,8 @@ constexpr size_t ws2_smem_bytes() {
 // MACC: the velocity-space moment of the new state is accumulated in registers over the vpar march (one
 // float2 per point of the thread); false for slabs too large for that (the host then runs gk_moment_kernel
 // on the new state).
-template <class ST, int NKY_, int NKX_, int NTF, int NTE, int NB, bool MACC = true>
+// CHI_ITEM: chis_cta is the base of a scratch indexed by (species, mu, s) instead of a per-CTA ring.
+template <class ST, int NKY_, int NKX_, int NTF, int NTE, int NB, bool MACC = true, bool CHI_ITEM = false>
 __device__ __forceinline__ void ws_epilogue_role2(const GkDev &P, const GkStageArgs &A, float2 *chis_cta,
                                                   const float2 *nl_cta, float *eblk, int tid) {
   constexpr int NT = NTF + NTE;
@@ -138,7 +139,8 @@ __device__ __forceinline__ void ws_epilogue_role2(const GkDev &P, const GkStageA
     const int al = w / (P.ns * P.nchunk);
     const int l = al % P.nmu, a = al / P.nmu;
     const long long base0 = (((long long)a * P.nv * P.nmu + l) * P.ns + i) * P.slab;
-    const float2 *chip = chis_cta + (it % GK_WS_CHI_RING) * 3 * slab + et;
+    const float2 *chip = (CHI_ITEM ? chis_cta + (((long long)a * P.nmu + l) * P.ns + i) * (3 * slab)
+                                   : chis_cta + (it % GK_WS_CHI_RING) * 3 * slab) + et;
     // without an FFT role the CTA builds chi and D_s chi itself; the first barrier below publishes them
     if constexpr (!NL) {
       build_chis(P, A, a, l, i, slab, nky, chis_cta + (it % GK_WS_CHI_RING) * 3 * slab, et, NTE);

@@ -40,9 +40,10 @@ gk_stage_ws3_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkS
   static_assert(NTF % 32 == 0 && NTE % 32 == 0, "roles are whole warps");
   constexpr int BAR_FFT = GK_WS_BAR_FFT, BAR_FULL = GK_WS_BAR_FULL, BAR_FREE = GK_WS_BAR_FREE;
   const int tid = threadIdx.x;
-  float2 *chis_cta = A.chis + (long long)blockIdx.x * (GK_WS_CHI_RING * 3 * slab);
+  // chi / D_s chi and grad(chi) live in scratch indexed by (species, mu, s), not by CTA: the CTAs that work on the
+  // vpar chunks of one (species, mu, s) at the same time write identical values and share the L2 lines
   float2 *nl_cta = A.nlbuf + (long long)blockIdx.x * (GK_WS_NL_RING * slab);
-  float2 *SGg = A.gchi + (long long)blockIdx.x * (MX_ * MY_);
+  float2 *SGg = A.gchi;
 
   float2 *XA = (float2 *)smem_raw;
   float2 *W = XA + MX_ * LDX;
@@ -260,7 +261,9 @@ gk_stage_ws3_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkS
       const int l = al % P.nmu, a = al / P.nmu;
       const long long base0 = (((long long)a * P.nv * P.nmu + l) * P.ns + i) * P.slab;
       const int j0 = c * P.jchunk, j1 = min(P.nv, (c + 1) * P.jchunk);
-      float2 *chis = chis_cta + (it % GK_WS_CHI_RING) * 3 * slab;
+      const long long item_li = ((long long)a * P.nmu + l) * P.ns + i;
+      float2 *chis = A.chis + item_li * (3 * slab);
+      SGg = A.gchi + item_li * (MX_ * MY_);
       build_chis(P, A, a, l, i, slab, NKY_, chis, tid, NTF);
       fsync();   // also: every thread has left the XF2 of the previous slab (XA is free)
       x1([&](int e) { return __ldcg(&chis[e]); });
@@ -299,7 +302,7 @@ gk_stage_ws3_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkS
     // consume the epilogue's last arrivals so that no barrier is left half-way at exit
     for (int v = max(0, u - GK_WS_NL_RING); v < u; ++v) bar_sync_n(BAR_FREE + (v & 1), NT);
   } else {
-    ws_epilogue_role2<ST, NKY_, NKX_, NTF, NTE, 1, false>(P, A, chis_cta, nl_cta, eblk, tid);
+    ws_epilogue_role2<ST, NKY_, NKX_, NTF, NTE, 1, false, true>(P, A, A.chis, nl_cta, eblk, tid);
   }
 }
 
