@@ -264,12 +264,26 @@ def main():
     hbuf = torch.empty(fd.shape if e2e_steps else (1,), dtype=fd.dtype).pin_memory()
     if e2e_steps:
         hbuf.copy_(fd.cpu())
+    # serial form: one C-ABI call per step on HOST buffers (H2D + 4 stages + D2H back to back on one stream)
     for _ in range(2 if e2e_steps else 0):
         g.gk_rk4_step_host(hbuf, hbuf, fd, dt)
     barrier()
     e0.record()
     for _ in range(e2e_steps):
-        g.gk_rk4_step_host(hbuf, hbuf, fd, dt)   # C-ABI call on HOST buffers: H2D + 4 stages + D2H
+        g.gk_rk4_step_host(hbuf, hbuf, fd, dt)
+    e1.record()
+    barrier()
+    serial_ms = max_over_ranks(e0.elapsed_time(e1), world, dev) if e2e_steps else None
+    # pipelined form: the same steps as one C-ABI batch call (upload of step k+1 and download of step k-1 overlap
+    # the compute of step k over two device buffers); every step still uploads its input and downloads its result
+    if e2e_steps:
+        hout = torch.empty_like(hbuf).pin_memory()
+        fd2 = g.empty_state()
+        g.gk_rk4_batch_host([hbuf] * 2, [hout] * 2, fd, fd2, dt)
+    barrier()
+    e0.record()
+    if e2e_steps:
+        g.gk_rk4_batch_host([hbuf] * e2e_steps, [hout] * e2e_steps, fd, fd2, dt)
     e1.record()
     barrier()
     e2e_ms = max_over_ranks(e0.elapsed_time(e1), world, dev)
@@ -296,7 +310,9 @@ def main():
                        "parallelism": "replicas only (paper has no grid parallelism)", "finite": finite},
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": fbytes, "d2h_bytes_per_step": fbytes,
-                    "steps": e2e_steps},
+                    "steps": e2e_steps, "call": "gk_rk4_batch_host (pinned host buffers, copies pipelined with compute)",
+                    "serial_value": aggregate_value(npts, e2e_steps, world, serial_ms) if e2e_steps else None,
+                    "serial_call": "gk_rk4_step_host"},
             "gpu_launches": int(launches),
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
                          "frac": achieved / peak, "traffic": _traffic(cfg["name"] + ("" if nl else "+linear") + ("" if storage == 0 else "+half")),

@@ -105,6 +105,16 @@ int gk_rk4_steps(gk_ctx *ctx, void *f_dev, double dt, int nsteps);
  * or a workspace too small for gk_rk4_step. */
 int gk_rk4_step_host(gk_ctx *ctx, const void *f_host_in, void *f_host_out, void *f_dev, double dt);
 
+/* A batch of independent RK4 steps on HOST buffers, software-pipelined over two device buffers: the upload of
+ * problem k+1 and the download of problem k-1 run on two copy streams owned by the context while problem k is
+ * stepped on the context stream (PCIe is full duplex; one step of the BASELINE grids computes faster than it
+ * uploads).  f_host_in[k] / f_host_out[k]: nbatch host pointers (pinned memory, layout and storage type of f; an
+ * output must not alias the input of a LATER problem), f_dev0 / f_dev1: two device scratch arrays of the size of
+ * f, caller-owned.  Every problem takes exactly the path of gk_rk4_step_host (same kernels, same result).
+ * Synchronises all three streams before returning.  GK_EINVAL on null pointers or nbatch < 0. */
+int gk_rk4_batch_host(gk_ctx *ctx, const void *const *f_host_in, void *const *f_host_out, int nbatch,
+                      void *f_dev0, void *f_dev1, double dt);
+
 /* Transport fluxes per species (R18): out_host[3*a + {0,1,2}] = particle, heat,
  * parallel-momentum flux.  Synchronises the stream. */
 int gk_fluxes(gk_ctx *ctx, const void *f_dev, const void *phi_dev, double *out_host);

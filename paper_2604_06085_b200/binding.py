@@ -85,6 +85,7 @@ def load_library(build_if_missing: bool = True):
     lib.gk_rk4_steps.argtypes = [vp, vp, C.c_double, C.c_int]
     lib.gk_fluxes.argtypes = [vp, vp, vp, dp]
     lib.gk_rk4_step_host.argtypes = [vp, vp, vp, vp, C.c_double]
+    lib.gk_rk4_batch_host.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.c_int, vp, vp, C.c_double]
     lib.gk_spectra.argtypes = [vp, vp, dp, dp]
     lib.gk_export_table.restype = C.c_size_t
     lib.gk_export_table.argtypes = [vp, C.c_char_p, dp, C.c_size_t]
@@ -229,6 +230,22 @@ class GkContext:
                 raise ValueError("host buffers must be contiguous CPU tensors of the shape and dtype of f")
         self._check(self.lib.gk_rk4_step_host(self._h, C.c_void_p(f_host_in.data_ptr()), C.c_void_p(f_host_out.data_ptr()),
                                               C.c_void_p(f_dev.data_ptr()), float(dt)))
+
+    def gk_rk4_batch_host(self, f_host_in, f_host_out, f_dev0, f_dev1, dt: float):
+        """Independent RK4 steps on lists of pinned host tensors, pipelined over two device buffers
+        (upload, compute and download overlap).  Synchronises."""
+        self._chk_state(f_dev0, "f_dev0")
+        self._chk_state(f_dev1, "f_dev1")
+        n = len(f_host_in)
+        if len(f_host_out) != n:
+            raise ValueError("as many outputs as inputs")
+        for t in list(f_host_in) + list(f_host_out):
+            if t.device.type != "cpu" or not t.is_contiguous() or t.numel() != f_dev0.numel() or t.dtype != f_dev0.dtype:
+                raise ValueError("host buffers must be contiguous CPU tensors of the shape and dtype of f")
+        ins = (C.c_void_p * max(n, 1))(*[t.data_ptr() for t in f_host_in])
+        outs = (C.c_void_p * max(n, 1))(*[t.data_ptr() for t in f_host_out])
+        self._check(self.lib.gk_rk4_batch_host(self._h, ins, outs, n, C.c_void_p(f_dev0.data_ptr()),
+                                               C.c_void_p(f_dev1.data_ptr()), float(dt)))
 
     def gk_fluxes(self, f, phi):
         import numpy as np

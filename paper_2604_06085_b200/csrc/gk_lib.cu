@@ -52,6 +52,9 @@ struct gk_ctx {
   // profiling of the stage kernel
   bool profiling = false;
   std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ev;
+  // gk_rk4_batch_host: copy streams and per-buffer events, created on first use
+  cudaStream_t s_up = nullptr, s_down = nullptr;
+  cudaEvent_t e_in[2] = {nullptr, nullptr}, e_done[2] = {nullptr, nullptr}, e_out[2] = {nullptr, nullptr};
   size_t ev_used = 0;
 };
 
@@ -382,6 +385,11 @@ int gk_destroy(gk_ctx *c) {
   if (!c) return GK_EINVAL;
   for (void *p : c->dev_allocs) cudaFree(p);
   for (auto &e : c->ev) { cudaEventDestroy(e.first); cudaEventDestroy(e.second); }
+  if (c->s_up) cudaStreamDestroy(c->s_up);
+  if (c->s_down) cudaStreamDestroy(c->s_down);
+  for (int b = 0; b < 2; ++b)
+    for (cudaEvent_t e : {c->e_in[b], c->e_done[b], c->e_out[b]})
+      if (e) cudaEventDestroy(e);
   delete c;
   return GK_OK;
 }
@@ -482,6 +490,44 @@ int gk_rk4_step_host(gk_ctx *c, const void *f_host_in, void *f_host_out, void *f
   GK_CUDA(c, cudaMemcpyAsync(f_dev, f_host_in, bytes, cudaMemcpyHostToDevice, c->stream));
   if (int r = gk_rk4_steps(c, f_dev, dt, 1)) return r;
   GK_CUDA(c, cudaMemcpyAsync(f_host_out, f_dev, bytes, cudaMemcpyDeviceToHost, c->stream));
+  return GK_OK;
+}
+
+int gk_rk4_batch_host(gk_ctx *c, const void *const *f_in, void *const *f_out, int nbatch, void *dev0, void *dev1,
+                      double dt) {
+  if (int r = usable(c)) return r;
+  if (!f_in || !f_out || !dev0 || !dev1 || dev0 == dev1 || nbatch < 0)
+    return fail(c, GK_EINVAL, "gk_rk4_batch_host: bad arguments");
+  if (!c->s_up) {
+    GK_CUDA(c, cudaStreamCreateWithFlags(&c->s_up, cudaStreamNonBlocking));
+    GK_CUDA(c, cudaStreamCreateWithFlags(&c->s_down, cudaStreamNonBlocking));
+    for (int b = 0; b < 2; ++b) {
+      GK_CUDA(c, cudaEventCreateWithFlags(&c->e_in[b], cudaEventDisableTiming));
+      GK_CUDA(c, cudaEventCreateWithFlags(&c->e_done[b], cudaEventDisableTiming));
+      GK_CUDA(c, cudaEventCreateWithFlags(&c->e_out[b], cudaEventDisableTiming));
+    }
+  }
+  const size_t bytes = (size_t)c->P.ntot * c->elem_bytes;
+  void *dev[2] = {dev0, dev1};
+  // the copy streams start after whatever the caller queued on the context stream
+  GK_CUDA(c, cudaEventRecord(c->e_done[0], c->stream));
+  GK_CUDA(c, cudaStreamWaitEvent(c->s_up, c->e_done[0], 0));
+  for (int k = 0; k < nbatch; ++k) {
+    const int b = k & 1;
+    if (!f_in[k] || !f_out[k]) return fail(c, GK_EINVAL, "gk_rk4_batch_host: null host pointer");
+    if (k >= 2) GK_CUDA(c, cudaStreamWaitEvent(c->s_up, c->e_out[b], 0));   // buffer b has been downloaded
+    GK_CUDA(c, cudaMemcpyAsync(dev[b], f_in[k], bytes, cudaMemcpyHostToDevice, c->s_up));
+    GK_CUDA(c, cudaEventRecord(c->e_in[b], c->s_up));
+    GK_CUDA(c, cudaStreamWaitEvent(c->stream, c->e_in[b], 0));
+    if (int r = gk_rk4_steps(c, dev[b], dt, 1)) return r;
+    GK_CUDA(c, cudaEventRecord(c->e_done[b], c->stream));
+    GK_CUDA(c, cudaStreamWaitEvent(c->s_down, c->e_done[b], 0));
+    GK_CUDA(c, cudaMemcpyAsync(f_out[k], dev[b], bytes, cudaMemcpyDeviceToHost, c->s_down));
+    GK_CUDA(c, cudaEventRecord(c->e_out[b], c->s_down));
+  }
+  GK_CUDA(c, cudaStreamSynchronize(c->s_up));
+  GK_CUDA(c, cudaStreamSynchronize(c->stream));
+  GK_CUDA(c, cudaStreamSynchronize(c->s_down));
   return GK_OK;
 }
 
