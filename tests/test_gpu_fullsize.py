@@ -121,3 +121,54 @@ def test_repeated_runs_are_bit_identical(n, linear):
         outs.append(fd)
     assert torch.equal(torch.view_as_real(outs[0]), torch.view_as_real(outs[1]))
     assert torch.equal(torch.view_as_real(outs[0]), torch.view_as_real(outs[2]))
+
+
+# The stage kernels are specialised on (padded grid, nkx, nky) only: a grid with the production (kx,ky)
+# plane and few points along s, vpar, mu runs exactly the production kernels (all RK modes, the register
+# / gk_moment_kernel moments that feed the next stage's field solve, the seam planes: 4 of 8 here) at a
+# size the oracle steps in seconds.
+SPECIALISED = {
+    "cfg2_plane": (dict(nkx=85, nky=16, ky0=0.07, ikxspace=5), 2),
+    "cfg3_plane": (dict(nkx=85, nky=32, ky0=0.035, ikxspace=5), 2),
+    "cfg5_plane": (dict(nkx=127, nky=64, ky0=0.0175, ikxspace=5), 4),
+}
+
+
+@pytest.mark.parametrize("case", ["cfg2_plane", "cfg3_plane", "cfg5_plane", "cfg3_plane_kinetic", "cfg3_plane_linear",
+                                  "cfg5_plane_f16"])
+def test_rk4_steps_parity_on_the_production_kernels(case):
+    import torch
+    from paper_2604_06085_b200 import GkContext
+    from tests.util import small_cfg, rand_c
+    base = case.replace("_kinetic", "").replace("_linear", "").replace("_f16", "")
+    grid, kind = SPECIALISED[base]
+    kw = dict(ns=8, nvpar=8, nmu=2, mu_grid=1, **grid)
+    if case.endswith("_kinetic"):
+        kw.update(nspecies=2, adiabatic=0, ky0=0.2)     # DESIGN.md R5: stable k_perp,min with kinetic electrons
+    cfg = small_cfg(**kw)
+    dt, nsteps = (0.0005, 2) if case.endswith("_kinetic") else (0.01, 3)
+    if case.endswith("_linear"):
+        cfg["opts"]["nonlinear"] = 0
+        kind = 3
+    if case.endswith("_f16"):
+        cfg["opts"]["storage"] = 1
+    g = GkContext(cfg)
+    assert g.plan()["kind"] == kind, g.plan()
+    o = GkRef(cfg)
+    # white noise of amplitude 0.03 in every mode: the bracket is a few per cent of the increment and the three
+    # steps stay bounded (amplitude 0.1 blows up within three steps, in the oracle as on the device)
+    amp = 0.003 if case.endswith("_kinetic") else 0.03
+    f = (rand_c(np.random.default_rng(61), o.shape, True) * amp).astype(np.complex64)
+    fd = g.to_state(f)
+    f0 = g.from_state(fd).astype(np.complex128)         # what the device holds (rounded for half storage)
+    g.gk_rk4_steps(fd, dt, nsteps)
+    torch.cuda.synchronize()
+    got = g.from_state(fd).astype(np.complex128)
+    ref = o.rk4_step(f0, dt, nsteps)
+    assert np.isfinite(ref).all() and np.abs(ref).max() < 10 * np.abs(f0).max()
+    if case.endswith("_f16"):
+        assert rel_l2(got, ref) < 1e-2
+    else:
+        assert rel_l2(got, ref) < 1e-4                   # north_star: 1e-4 after RK4 steps
+        # the increment itself (not masked by f0): fp32 rounding of f1 - f0 is ~1e-6 of it
+        assert rel_l2(got - f0, ref - f0) < 2e-5, rel_l2(got - f0, ref - f0)
