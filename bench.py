@@ -188,6 +188,67 @@ def run_reference(args, cfg, rank):
     print(json.dumps(line), flush=True)
 
 
+def run_cufft_compare(args, cfg):
+    """Measured comparison only (north_star: cuFFT is allowed as a measured comparison): term III of
+    one stage done the library way -- padded gradient spectra written to HBM, batched cuFFT c2r (torch.fft.irfft2),
+    pointwise product, cuFFT r2c, truncation -- on arrays of the workload's shape, beside the fused stage kernel.
+    The ky=0 Hermitian average (R15) is not applied here: this is a timing of the data movement, not a parity path."""
+    import torch
+    from paper_2604_06085_b200 import GkContext
+    dev = torch.device("cuda", 0)
+    g = GkContext(cfg, device=dev)
+    nsp, nv, nmu, ns, nkx, nky = g.shape
+    K = (nkx - 1) // 2
+    plan = g.plan()
+    mx, my = plan["mx"], plan["my"]
+    nli = 8                                   # (mu, s) pairs per batch: nli * nv slabs
+    nbatch = (nsp * nmu * ns + nli - 1) // nli
+    gen = torch.Generator(device=dev).manual_seed(1)
+    f = torch.randn(nli, nv, nkx, nky, 2, device=dev, generator=gen)
+    f = torch.view_as_complex(f) * 1e-3
+    gchi = torch.randn(2, nli, 1, mx, my, device=dev, generator=gen)   # real-space grad(chi), reused over vpar
+    kx = (torch.arange(nkx, device=dev) - K).float().view(1, 1, nkx, 1) * 0.1
+    ky = torch.arange(nky, device=dev).float().view(1, 1, 1, nky) * 0.1
+    pad = torch.zeros(2, nli, nv, mx, my // 2 + 1, dtype=torch.complex64, device=dev)
+
+    def bracket_batch():
+        gx, gy = 1j * kx * f, 1j * ky * f
+        for q, src in enumerate((gx, gy)):
+            pad[q, :, :, :K + 1, :nky] = src[:, :, K:, :]
+            pad[q, :, :, mx - K:, :nky] = src[:, :, :K, :]
+        real = torch.fft.irfft2(pad, s=(mx, my), norm="forward")
+        br = gchi[1] * real[0] - gchi[0] * real[1]
+        out = torch.fft.rfft2(br, norm="forward")
+        return torch.cat((out[:, :, mx - K:, :nky], out[:, :, :K + 1, :nky]), dim=2)
+
+    for _ in range(3):
+        bracket_batch()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    reps = max(1, args.steps)
+    e0.record()
+    for _ in range(reps * nbatch):
+        bracket_batch()
+    e1.record()
+    torch.cuda.synchronize()
+    ms_stage = e0.elapsed_time(e1) / reps
+    # the fused stage kernel (whole stage: field solve + linear terms + bracket + RK update) on the same grid
+    fd = g.to_state(gkinputs.initial_f(cfg, np.complex64))
+    g.gk_rk4_steps(fd, cfg["dt"], 3)
+    torch.cuda.synchronize()
+    e0.record()
+    g.gk_rk4_steps(fd, cfg["dt"], reps)
+    e1.record()
+    torch.cuda.synchronize()
+    fused = e0.elapsed_time(e1) / (4 * reps)
+    print(json.dumps({"compare": "cufft_unfused_bracket", "workload": cfg["name"], "padded_fft": [mx, my],
+                      "slabs_per_stage": nsp * nv * nmu * ns, "batch_slabs": nli * nv,
+                      "cufft_bracket_ms_per_stage": ms_stage, "fused_whole_stage_ms": fused,
+                      "ratio_bracket_alone_over_whole_fused_stage": ms_stage / fused,
+                      "note": "torch.fft (cuFFT) irfft2/rfft2 with padded arrays in HBM; term III only, no linear terms, "
+                              "no RK update, no field solve"}), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -199,6 +260,7 @@ def main():
     ap.add_argument("--linear", action="store_true", help="switch term III off (HBM-bound variant)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs)")
+    ap.add_argument("--compare", default=None, choices=["cufft"], help="measured comparison: term III through cuFFT, unfused")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "gk" else args.warmup
 
@@ -209,6 +271,10 @@ def main():
         run_reference(args, replica_config(args.config, 0, args.storage, args.linear), rank)
         return
     cfg = replica_config(args.config, rank, args.storage, args.linear)
+    if args.compare == "cufft":
+        if rank == 0:
+            run_cufft_compare(args, cfg)
+        return
 
     import torch
     import torch.distributed as dist
