@@ -394,6 +394,12 @@ gk_stage_ws2_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkS
     // =============================== FFT role =====================================
     if constexpr (RF > 0) asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(RF));
     const gkfft::NamedSync<BAR_FFT, NTF> fsync;
+    // With 512 FFT threads and mx = 128 the item maps below keep two groups of warps (even / odd warp index)
+    // closed under Y1 -> YF -> F2 (rows p, p + H with p < 32 / p >= 32) and, when a warp spans 32 of the 2 nky
+    // columns, under X1 -> X2 (P / Q columns): those hand-offs need only a barrier among the 256 threads of a
+    // group, and the two groups drift apart and fill each other's latency gaps.
+    constexpr bool GRP = (NTF == 512 && MX_ == 128), GRPX = GRP && (NC == 64);
+    auto gsync = [&]() { asm volatile("bar.sync %0, %1;" ::"r"(6 + ((tid >> 5) & 1)), "n"(NTF / 2) : "memory"); };
     // ---- X1: inverse x pass 1 of the spectral slab g (callable: slab index -> value) ----
     auto x1 = [&](auto g) {
       for (int w = tid; w < NC * RX1; w += NTF) {
@@ -652,15 +658,16 @@ gk_stage_ws2_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkS
         mbar_wait(mbar, parity);
         parity ^= 1u;
         x1([&](int e) { return Cv<ST>::ld(stg, e); });
-        fsync();
-        if (tid == 0 && j + 1 < j1)
-          bulk_load(stg, (const ST *)A.y + (base0 + (long long)(j + 1) * jstride), slab * sizeof(ST), mbar);
+        if constexpr (GRPX) gsync(); else fsync();
         x2();
         fsync();
+        // every thread has left X1: the staging buffer may take the next slab
+        if (tid == 0 && j + 1 < j1)
+          bulk_load(stg, (const ST *)A.y + (base0 + (long long)(j + 1) * jstride), slab * sizeof(ST), mbar);
         y1();
-        fsync();
+        if constexpr (GRP) gsync(); else fsync();
         yf();
-        fsync();
+        if constexpr (GRP) gsync(); else fsync();
         f2();
         fsync();
         xf1();
