@@ -70,7 +70,8 @@ template <class ST> StagePick pick_stage_ws2(int mx, int my, int nky, int nkx, i
     return {(const void *)gk::gk_stage_ws2_kernel<ST, MX, MY, NKY, NKX, NTF, NTE, RF, RE, NB>, NTF + NTE, 1, NTF, \
             gk::ws2_smem_bytes<ST, MX, MY, NKY, NKX>(), 2}
   // measured on B200, cfg3 (ms per stage): 512+384 threads 1.42, 512+256 (2 points in flight) 1.42-1.43,
-  // 768+256 1.48, 512+512 without setmaxnreg 1.84; the forward-x pass 2 moved into the epilogue role 1.44-1.53
+  // 768+256 1.46-1.48 (48/112 and 40/136 registers), 512+512 without setmaxnreg 1.84; the forward-x pass 2 moved
+  // into the epilogue role 1.44-1.53
   GK_WS2(512, 128, 96, 32, 85, 512, 384, 56, 88, 1);
   GK_WS2(513, 128, 96, 32, 85, 512, 256, 56, 128, 2);
   GK_WS2(512, 128, 48, 16, 85, 512, 384, 56, 88, 1);
