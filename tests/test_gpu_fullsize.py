@@ -99,7 +99,7 @@ def test_config5_half_storage_against_complex64_run():
     assert rel_l2(out16, out32) < 1e-2
 
 
-@pytest.mark.parametrize("n,linear", [(2, False), (3, False), (3, True)])
+@pytest.mark.parametrize("n,linear", [(2, False), (3, False), (3, True), (5, False)])
 def test_repeated_runs_are_bit_identical(n, linear):
     # The stage kernels use no atomics: every output has one writer and a fixed summation order, and the
     # roles of the warp-specialised kernels hand data over through named barriers, an mbarrier and L2
