@@ -10,6 +10,7 @@
  *          from -K to K, ky index m = 0..nky-1 (half spectrum, ky_m = m*ky0).
  *          storage 0: complex64 (float re, float im); 1: complex fp16 (__half2); 2: complex bf16.
  *   - phi: [s i][kx p+K][ky m] complex64, always.
+ *   - f, rhs and the host-call device buffers must be 16-byte aligned (slabs move by bulk copies): GK_EINVAL.
  *   - Caller owns f, phi, rhs and the workspace; the context owns only its coefficient tables.
  *   - Hot calls (field_solve, rhs, rk4_step, rk4_steps) are asynchronous on the stream given to
  *     gk_create, never synchronise and never allocate.  gk_fluxes synchronises the stream.

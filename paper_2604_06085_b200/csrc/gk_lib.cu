@@ -418,6 +418,7 @@ int gk_field_solve(gk_ctx *c, const void *f, void *phi) {
 int gk_rhs(gk_ctx *c, const void *f, void *phi, void *rhs) {
   if (int r = usable(c)) return r;
   if (!f || !phi || !rhs || rhs == f || !c->ws) return fail(c, GK_EINVAL, "gk_rhs: bad pointers or no workspace");
+  if (((uintptr_t)f | (uintptr_t)rhs) & 15) return fail(c, GK_EINVAL, "gk_rhs: f and rhs must be 16-byte aligned");
   if (int r = gk_field_solve(c, f, phi)) return r;
   GkStageArgs A;
   std::memset(&A, 0, sizeof(A));
@@ -433,6 +434,7 @@ int gk_rhs(gk_ctx *c, const void *f, void *phi, void *rhs) {
 int gk_rk4_steps(gk_ctx *c, void *f, double dt, int nsteps) {
   if (int r = usable(c)) return r;
   if (!f || !c->ws || nsteps < 0) return fail(c, GK_EINVAL, "gk_rk4_steps: bad arguments or no workspace");
+  if ((uintptr_t)f & 15) return fail(c, GK_EINVAL, "gk_rk4_steps: f must be 16-byte aligned (bulk copies of whole slabs)");
   if (c->ws_bytes < c->need_full) return fail(c, GK_EINVAL, "workspace too small for gk_rk4_step");
   char *ws = (char *)c->ws;
   float2 *mom = (float2 *)(ws + c->off_mom);
