@@ -383,7 +383,7 @@ def main():
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
                          "frac": achieved / peak, "traffic": _traffic(cfg["name"] + ("" if nl else "+linear") + ("" if storage == 0 else "+half")),
                          "traffic_unit": "GB of DRAM read+write per stage-kernel launch (ncu, profiles/)", "peak_source": peak_src,
-                         "kernel": ["gk_stage_kernel", "gk_stage_ws_kernel", "gk_stage_ws2_kernel", "gk_stage_lin_kernel", "gk_stage_ws3_kernel"][plan.get("kind", 0)], "launches_timed": int(stage_n),
+                         "kernel": {0: "gk_stage_kernel", 2: "gk_stage_ws2_kernel", 3: "gk_stage_lin_kernel", 5: "gk_stage_ws4_kernel"}[plan["kind"]], "launches_timed": int(stage_n),
                          "avg_launch_ms": stage_avg_ms, "alg_bytes_per_point": bpp,
                          "stage_share_of_step": stage_ms / ms if ms > 0 else None},
         }

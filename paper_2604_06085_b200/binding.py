@@ -291,5 +291,5 @@ class GkContext:
     def plan(self) -> dict:
         p = self.gk_export_table("pad")
         return dict(mx=int(p[0]), my=int(p[1]), rc=int(p[2]), gchi_in_smem=int(p[3]), jchunk=int(p[4]),
-                    nchunk=int(p[5]), stage_grid=int(p[6]), stage_smem=int(p[7]), threads=int(p[8]), occ=int(p[9]),
-                    ws=int(p[10]) if len(p) > 10 else 0, kind=int(p[11]) if len(p) > 11 else 0)
+                    nchunk=int(p[5]), stage_grid=int(p[6]), stage_smem=int(p[7]), threads=int(p[8]), cluster=int(p[9]),
+                    nsh=int(p[10]), kind=int(p[11]))

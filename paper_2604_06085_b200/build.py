@@ -21,14 +21,12 @@ UNITS = [
     ("gk_stage_inst.cu", ["-DGK_ST_ID=1"], "gk_stage_f16.o"),
     ("gk_stage_inst.cu", ["-DGK_ST_ID=2"], "gk_stage_bf16.o"),
 ]
-DEPS = ["gk_lib.cu", "gk_stage_inst.cu", "gk_kernels.cuh", "gk_common.cuh", "gk_stage.cuh", "gk_stage_ws.cuh", "gk_stage_ws2.cuh", "gk_fft.cuh", "gk_tables.h",
-        "gk_dev.h", "gk_pick.h"]
-# per translation unit: a unit is recompiled only if its object is older than one of these
-UNIT_DEPS = {
-    "gk_lib.cu": ["gk_lib.cu", "gk_kernels.cuh", "gk_common.cuh", "gk_fft.cuh", "gk_tables.h", "gk_dev.h", "gk_pick.h"],
-    "gk_stage_inst.cu": ["gk_stage_inst.cu", "gk_common.cuh", "gk_stage.cuh", "gk_stage_ws.cuh", "gk_stage_ws2.cuh",
-                         "gk_fft.cuh", "gk_dev.h", "gk_pick.h"],
-}
+
+
+def _csrc_files():
+    """Every translation unit includes (directly or not) every header of csrc/: one dependency list."""
+    return sorted(os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".cu", ".cuh", ".h")))
+
 
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
@@ -43,12 +41,23 @@ def _nvcc() -> str:
     return "nvcc"
 
 
+def _flags_now() -> str:
+    fast = bool(os.environ.get("GK_FAST_BUILD"))           # developer builds only: complex64 storage
+    return " ".join([*NVCC_FLAGS, *(["-DGK_ONLY_C64"] if fast else [])])
+
+
+def _include_files():
+    return sorted(os.path.join(INCLUDE, f) for f in os.listdir(INCLUDE) if f.endswith(".h"))
+
+
 def is_stale() -> bool:
-    if not os.path.exists(LIB):
+    """The library is rebuilt if it is missing, older than any file of csrc/ or include/, or was built with
+    other flags (GK_FAST_BUILD)."""
+    flagfile = os.path.join(OBJDIR, "flags.txt")
+    if not os.path.exists(LIB) or not os.path.exists(flagfile) or open(flagfile).read() != _flags_now():
         return True
     t = os.path.getmtime(LIB)
-    deps = [os.path.join(CSRC, d) for d in DEPS] + [os.path.join(INCLUDE, "gk.h")]
-    return any(os.path.getmtime(d) > t for d in deps)
+    return any(os.path.getmtime(d) > t for d in _csrc_files() + _include_files())
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
@@ -62,14 +71,14 @@ def build(force: bool = False, verbose: bool = False) -> str:
     extra = ["-DGK_ONLY_C64"] if fast else []
 
     flagfile = os.path.join(OBJDIR, "flags.txt")
-    flags_now = " ".join([*NVCC_FLAGS, *extra])
+    flags_now = _flags_now()
     same_flags = os.path.exists(flagfile) and open(flagfile).read() == flags_now
 
     def compile_unit(u):
         src, defs, obj = u
         objp = os.path.join(OBJDIR, obj)
         cmd = [_nvcc(), *NVCC_FLAGS, *extra, *defs, "-c", os.path.join(CSRC, src), "-o", objp]
-        deps = [os.path.join(CSRC, d) for d in UNIT_DEPS[src]] + [os.path.join(INCLUDE, "gk.h")]
+        deps = _csrc_files() + _include_files()
         if not force and same_flags and os.path.exists(objp) and all(os.path.getmtime(d) <= os.path.getmtime(objp) for d in deps):
             return cmd, subprocess.CompletedProcess(cmd, 0, "(up to date)\n", "")
         res = subprocess.run(cmd, capture_output=True, text=True)

@@ -51,4 +51,12 @@ template <> struct Cv<__nv_bfloat162> {
   static __device__ __forceinline__ void stcs(void *p, long long i, float2 v) { __stcs((__nv_bfloat162 *)p + i, __float22bfloat162_rn(v)); }
 };
 
+// the value a stored number has when it is read back (identity for complex64): the moment of the new state is
+// accumulated from what the next stage will actually read
+template <class ST> __device__ __forceinline__ float2 as_stored(float2 v) { return v; }
+template <> __device__ __forceinline__ float2 as_stored<__half2>(float2 v) { return __half22float2(__float22half2_rn(v)); }
+template <> __device__ __forceinline__ float2 as_stored<__nv_bfloat162>(float2 v) {
+  return __bfloat1622float2(__float22bfloat162_rn(v));
+}
+
 }  // namespace gk

@@ -3,6 +3,8 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <new>
+#include <stdexcept>
 #include <string>
 #include <vector>
 
@@ -37,15 +39,15 @@ struct gk_ctx {
   bool poisoned = false;
   int num_sms = 0;
   int stage_grid = 0;
-  int stage_threads = 512, stage_occ = 1, stage_ws = 0, stage_kind = 0, host_moment = 0;
-  size_t stage_gchi = 0;
+  int stage_threads = 512, stage_kind = 0, stage_cluster = 1, stage_nsh = 1;
   size_t stage_smem = 0;
   size_t elem_bytes = 8;
   // workspace
   void *ws = nullptr;
   size_t ws_bytes = 0;
   size_t off_mom = 0, off_phi = 0, off_gchi = 0, off_chis = 0, off_nl = 0, off_ya = 0, off_yb = 0, off_acc = 0;
-  const void *stage_fn = nullptr;  // the gk_stage_kernel instantiation chosen at create time
+  const void *stage_fn = nullptr;  // the stage-kernel instantiation chosen at create time
+  int stage_nwork = 0;
   size_t need_rhs = 0, need_full = 0;
   bool mom_valid_for_f = false;  // inside gk_rk4_steps only
   long long launches = 0;
@@ -104,9 +106,28 @@ template <class ST> void launch_moment(gk_ctx *c, const void *f, float2 *mom) {
   ++c->launches;
 }
 
+void stage_config(const gk_ctx *c, cudaLaunchConfig_t &cfg, cudaLaunchAttribute &attr) {
+  std::memset(&cfg, 0, sizeof(cfg));
+  cfg.gridDim = dim3(c->stage_grid);
+  cfg.blockDim = dim3(c->stage_threads);
+  cfg.dynamicSmemBytes = c->stage_smem;
+  cfg.stream = c->stream;
+  if (c->stage_cluster > 1) {   // thread-block cluster: the CTAs of a cluster share one work item
+    attr.id = cudaLaunchAttributeClusterDimension;
+    attr.val.clusterDim.x = c->stage_cluster;
+    attr.val.clusterDim.y = 1;
+    attr.val.clusterDim.z = 1;
+    cfg.attrs = &attr;
+    cfg.numAttrs = 1;
+  }
+}
+
 void launch_stage(gk_ctx *c, const GkStageArgs &A) {
   void *args[2] = {(void *)&c->P, (void *)&A};
-  cudaLaunchKernel(c->stage_fn, dim3(c->stage_grid), dim3(c->stage_threads), args, c->stage_smem, c->stream);
+  cudaLaunchConfig_t cfg;
+  cudaLaunchAttribute attr;
+  stage_config(c, cfg, attr);
+  cudaLaunchKernelExC(&cfg, c->stage_fn, args);
   ++c->launches;
 }
 
@@ -176,8 +197,12 @@ const char *gk_version(void) { return "gk-b200 0.1 (sm_100a)"; }
 
 const char *gk_last_error(const gk_ctx *c) { return c ? c->err.c_str() : "null context"; }
 
-int gk_create(const gk_grid *g, const gk_species *sp, const gk_salpha *geo, const gk_opts *o,
-              void *cuda_stream, gk_ctx **out) {
+}  // extern "C"
+
+namespace {
+
+int create_impl(const gk_grid *g, const gk_species *sp, const gk_salpha *geo, const gk_opts *o,
+                void *cuda_stream, gk_ctx **out) {
   if (!g || !sp || !geo || !o || !out) return GK_EINVAL;
   *out = nullptr;
   if (g->nkx < 1 || g->nkx % 2 == 0 || g->ns < 4 || g->nvpar < 4 || g->nky < 1 || g->nmu < 1 ||
@@ -236,106 +261,100 @@ int gk_create(const gk_grid *g, const gk_species *sp, const gk_salpha *geo, cons
   for (int q = 0; q < 50; ++q) (&P.dcoef[0][0][0])[q] = (float)(&T.dcoef[0][0][0])[q];
   for (int q = 0; q < 25; ++q) (&P.discoef[0][0])[q] = (float)(&T.discoef[0][0])[q];
 
-  // padded grid of the bracket (3/2 rule; R14)
-  const int need_x = 3 * T.K + 1, need_y = 3 * (T.nky - 1) + 1;
-  P.mx = o->pad_mx > 0 ? o->pad_mx : smallest_pad(std::max(need_x, 2));
-  P.my = o->pad_my > 0 ? o->pad_my : smallest_pad(std::max(need_y, 2));
+  // padded grid of the bracket (3/2 rule; R14); without term III no padded grid exists
   const bool nl = (P.mask & GK_T_III) != 0;
+  const int need_x = 3 * T.K + 1, need_y = 3 * (T.nky - 1) + 1;
   if (nl) {
+    P.mx = o->pad_mx > 0 ? o->pad_mx : smallest_pad(std::max(need_x, 2));
+    P.my = o->pad_my > 0 ? o->pad_my : smallest_pad(std::max(need_y, 2));
     if (P.mx < need_x || P.my < need_y || !gkfft::supported_len(P.mx) || !gkfft::supported_len(P.my))
       return fail(c, GK_EUNSUPPORTED, "padded grid must be 2^a*3^b (b<=1), <=256 and satisfy the 3/2 rule");
     if (P.mx % 2) return fail(c, GK_EUNSUPPORTED, "padded x size must be even (row pairs)");
+  } else {
+    P.mx = P.my = 2;
   }
   P.fftnorm = (float)(1.0 / ((double)P.mx * P.my));
   P.prefetch = 1;
-  if (const char *env = std::getenv("GK_PREFETCH")) P.prefetch = std::atoi(env);
   P.ldx = 2 * T.nky + 1;
   P.ldy = P.my | 1;
 
-  // Kernel variant: (threads per CTA, CTAs per SM) by measured preference; GK_STAGE_THREADS and
-  // GK_STAGE_OCC override the choice (tuning knobs).  A variant whose shared-memory plan needs
-  // grad(chi) spilled to global scratch at occ = 2 is skipped in favour of one CTA per SM.
-  int force_occ = 0, force_thr = 0;
-  if (const char *env = std::getenv("GK_STAGE_OCC")) force_occ = std::atoi(env);
-  if (const char *env = std::getenv("GK_STAGE_THREADS")) force_thr = std::atoi(env);
-  // warp-specialised kernel (FFT warps + epilogue warps): GK_WS_NTF = FFT-role threads, 0 = unified kernel
-  int ws_ntf = 512;
-  if (const char *env = std::getenv("GK_WS_NTF")) ws_ntf = std::atoi(env);
-  if (force_occ || force_thr) ws_ntf = 0;
-  long long nwork = 0;
-  for (int attempt = 0; attempt < 2; ++attempt) {
-    StagePick pick;
-    pick = gk_pick_stage(o->storage, P.mx, P.my, P.nky, P.nkx, nl, force_occ, force_thr, ws_ntf);
-    if (!pick.fn) return fail(c, GK_EUNSUPPORTED, "this build has no stage kernel for the requested storage");
-    c->stage_fn = pick.fn;
-    c->stage_threads = pick.threads;
-    c->stage_occ = pick.occ;
-    c->stage_ws = pick.ws;
-    c->stage_kind = pick.kind;
-    c->host_moment = pick.host_moment;
-    c->stage_gchi = pick.gchi;
-    const int resident = c->num_sms * pick.occ;  // persistent CTAs
-
-    // work decomposition: items (a, l, vpar chunk, i) are dealt round-robin to the persistent CTAs.
-    // Cost of a split = rounds x (slabs per item + the chi build of the item, in slab units);
-    // chunks stay >= 4 long so that chi is amortised.
-    {
-      const long long ali = (long long)T.nsp * T.nmu * T.ns;
-      const double chi_cost = nl ? 0.7 : 0.3;
-      double best = 1e300;
-      for (int nch = 1; nch <= std::max(1, T.nv / 4); ++nch) {
-        const int jc = (T.nv + nch - 1) / nch;
-        const int nce = (T.nv + jc - 1) / jc;
-        const long long rounds = (ali * nce + resident - 1) / resident;
-        const double cost = (double)rounds * (jc + chi_cost);
-        if (cost < best - 1e-9) { best = cost; P.jchunk = jc; P.nchunk = nce; }
-      }
-      P.nparts = T.nsp * T.nmu * P.nchunk;
-    }
-    nwork = (long long)T.nsp * T.nmu * T.ns * P.nchunk;
-
-    // shared-memory plan (per CTA: the SM's 227 KB opt-in capacity / occ, minus 1 KB reserved per CTA)
-    if (nl && pick.smem) {  // in-place warp-specialised kernel: fixed plan
-      P.rc = P.mx;
-      P.gchi_in_smem = 1;
-      c->stage_smem = pick.smem;
-      c->stage_grid = (int)std::min<long long>(nwork, resident);
-    } else if (nl) {
-      const size_t cap = pick.occ == 1 ? kSmemMax : (kSmemMax + 1024) / pick.occ - 1024;
-      const size_t fixed = ((size_t)P.mx + P.my + (size_t)P.mx * P.ldx) * 8;
-      const size_t gbytes = (size_t)P.mx * P.ldy * 8;
-      int rc_best = 0, in_smem = 0;
-      for (int pass = 0; pass < 2 && !rc_best; ++pass) {
-        const size_t base = fixed + (pass == 0 ? gbytes : 0);
-        for (int rc = P.mx; rc >= 2; rc /= 2) {
-          if (P.mx % rc || rc % 2) continue;
-          if (base + (size_t)rc * P.ldy * 8 <= cap) {
-            // keep at least 16 rows per chunk while grad(chi) is resident, otherwise spill it
-            if (pass == 0 && rc < std::min(16, P.mx)) break;
-            rc_best = rc;
-            in_smem = (pass == 0);
-            break;
-          }
+  // Kernel by shape (gk_stage_inst.cu) and its launch plan.
+  const StagePick pick = gk_pick_stage(o->storage, P.mx, P.my, P.nky, P.nkx, nl);
+  if (!pick.fn) return fail(c, GK_EUNSUPPORTED, "this build has no stage kernel for the requested storage");
+  c->stage_fn = pick.fn;
+  c->stage_threads = pick.threads;
+  c->stage_kind = pick.kind;
+  c->stage_cluster = pick.cluster;
+  c->stage_nsh = pick.nsh;
+  P.rc = nl ? P.mx : 2;
+  P.gchi_in_smem = 1;
+  if (pick.kind == GK_KIND_GENERIC && nl) {
+    // shared-memory plan of the generic kernel: x-transformed spectra + a chunk of rc rows for the y transforms,
+    // grad(chi) in shared memory if it fits next to at least 16 rows, else in per-CTA global scratch
+    const size_t fixed = ((size_t)P.mx + P.my + (size_t)P.mx * P.ldx) * 8;
+    const size_t gbytes = (size_t)P.mx * P.ldy * 8;
+    int rc_best = 0, in_smem = 0;
+    for (int pass = 0; pass < 2 && !rc_best; ++pass) {
+      const size_t base = fixed + (pass == 0 ? gbytes : 0);
+      for (int rc = P.mx; rc >= 2; rc /= 2) {
+        if (P.mx % rc || rc % 2) continue;
+        if (base + (size_t)rc * P.ldy * 8 <= kSmemMax) {
+          if (pass == 0 && rc < std::min(16, P.mx)) break;
+          rc_best = rc;
+          in_smem = (pass == 0);
+          break;
         }
       }
-      if (pick.occ == 2 && !in_smem && attempt == 0 && !std::getenv("GK_STAGE_OCC")) { force_occ = 1; continue; }
-      if (!rc_best) return fail(c, GK_EUNSUPPORTED, "padded grid does not fit the shared-memory strategy");
-      P.rc = rc_best;
-      P.gchi_in_smem = in_smem;
-      c->stage_smem = fixed + (in_smem ? gbytes : 0) + (size_t)P.rc * P.ldy * 8;
-      c->stage_grid = (int)std::min<long long>(nwork, resident);
-    } else {
-      P.rc = 2;
-      P.gchi_in_smem = 1;
-      c->stage_smem = pick.kind == 3 ? 0 : (size_t)P.slab * 8;
-      c->stage_grid = (int)std::min<long long>(nwork, resident);
     }
-    break;
+    if (!rc_best) return fail(c, GK_EUNSUPPORTED, "padded grid does not fit the shared-memory strategy");
+    P.rc = rc_best;
+    P.gchi_in_smem = in_smem;
+    c->stage_smem = fixed + (in_smem ? gbytes : 0) + (size_t)P.rc * P.ldy * 8;
+  } else if (pick.kind == GK_KIND_GENERIC) {
+    c->stage_smem = (size_t)P.slab * 8;
+  } else {
+    c->stage_smem = pick.smem;
   }
   {
-    cudaError_t e = cudaFuncSetAttribute(c->stage_fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->stage_smem);
+    // The attribute belongs to the kernel symbol, not to this context: the generic kernel (one symbol, plan by
+    // shape) always gets the opt-in maximum so that contexts of different shapes can coexist.
+    const size_t attr_smem = pick.kind == GK_KIND_GENERIC ? kSmemMax : c->stage_smem;
+    cudaError_t e = cudaFuncSetAttribute(c->stage_fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)attr_smem);
     if (e != cudaSuccess) return fail(c, GK_ECUDA, std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e));
   }
+  // persistent launch: one CTA per SM, or as many clusters as the device keeps resident at once
+  int resident = c->num_sms;   // units that take one work item at a time (CTAs or clusters)
+  if (pick.cluster > 1) {
+    c->stage_grid = c->num_sms / pick.cluster * pick.cluster;
+    cudaLaunchConfig_t cfg;
+    cudaLaunchAttribute attr;
+    stage_config(c, cfg, attr);
+    int ncl = 0;
+    cudaError_t e = cudaOccupancyMaxActiveClusters(&ncl, c->stage_fn, &cfg);
+    if (e != cudaSuccess || ncl < 1)
+      return fail(c, GK_ECUDA, std::string("cudaOccupancyMaxActiveClusters: ") + cudaGetErrorString(e));
+    resident = std::min(ncl, c->num_sms / pick.cluster);
+  }
+  // work decomposition: items (a, l, vpar chunk, share, i) are dealt round-robin to the resident units.
+  // Cost of a split = rounds x (slabs per item + the per-item set-up in slab units: chi / grad(chi) build,
+  // and the 4 slabs that fill the vpar register window); chunks stay >= 4 long so that the set-up is amortised.
+  long long nwork = 0;
+  {
+    const long long ali = (long long)T.nsp * T.nmu * T.ns * pick.nsh;
+    const double setup = pick.kind == GK_KIND_LIN ? 1.5 : (pick.kind == GK_KIND_WS4 ? 1.7 : (nl ? 0.7 : 0.3));
+    double best = 1e300;
+    for (int nch = 1; nch <= std::max(1, T.nv / 4); ++nch) {
+      const int jc = (T.nv + nch - 1) / nch;
+      const int nce = (T.nv + jc - 1) / jc;
+      const long long rounds = (ali * nce + resident - 1) / resident;
+      const double cost = (double)rounds * (jc + setup);
+      if (cost < best - 1e-9) { best = cost; P.jchunk = jc; P.nchunk = nce; }
+    }
+    P.nparts = T.nsp * T.nmu * P.nchunk;
+    nwork = ali * P.nchunk;
+  }
+  c->stage_nwork = (int)nwork;
+  c->stage_grid = (int)std::min<long long>(nwork, resident) * pick.cluster;
 
   // tables -> device
   int rcode;
@@ -363,22 +382,43 @@ int gk_create(const gk_grid *g, const gk_species *sp, const gk_salpha *geo, cons
   c->off_mom = off; off += align256((size_t)P.nparts * P.nphi * 8);
   c->off_phi = off; off += align256((size_t)P.nphi * 8);
   c->off_gchi = off;
-  // gk_stage_ws3_kernel (kind 4): scratch per (species, mu, s), shared by the CTAs that work on its vpar chunks
-  const size_t n_li = (size_t)T.nsp * T.nmu * T.ns;
-  if (nl && c->stage_kind == 4) off += align256(n_li * c->stage_gchi * 8);
-  else if (nl && c->stage_gchi) off += align256((size_t)c->stage_grid * c->stage_gchi * 8);
-  else if (nl && !P.gchi_in_smem) off += align256((size_t)c->stage_grid * P.mx * P.ldy * 8);
-  c->off_chis = off;
-  if (c->stage_kind == 4) off += align256(n_li * 3 * P.slab * 8);
-  else off += align256((size_t)c->stage_grid * (c->stage_ws ? 9 : 3) * P.slab * 8);
-  c->off_nl = off;
-  if (c->stage_ws) off += align256((size_t)c->stage_grid * 2 * P.slab * 8);
+  if (nl && !P.gchi_in_smem) off += align256((size_t)c->stage_grid * P.mx * P.ldy * 8);
+  c->off_chis = off; off += align256((size_t)c->stage_grid * pick.chis_per_cta * 8);
+  c->off_nl = off; off += align256((size_t)c->stage_grid * pick.nl_per_cta * 8);
   c->need_rhs = off;
   c->off_ya = off; off += align256((size_t)P.ntot * c->elem_bytes);
   c->off_yb = off; off += align256((size_t)P.ntot * c->elem_bytes);
   c->off_acc = off; off += align256((size_t)P.ntot * c->elem_bytes);
   c->need_full = off;
   return GK_OK;
+}
+
+}  // namespace
+
+// No exception crosses the ABI: allocation failures of the host-side tables map to GK_ENOMEM, anything else
+// to GK_EINVAL (the context, if it was created, carries the text).
+#define GK_GUARDED(ctx, expr)                                                     \
+  try {                                                                           \
+    return (expr);                                                                \
+  } catch (const std::bad_alloc &) {                                              \
+    return fail(ctx, GK_ENOMEM, "out of host memory");                            \
+  } catch (const std::exception &e) {                                             \
+    return fail(ctx, GK_EINVAL, std::string("internal error: ") + e.what());      \
+  } catch (...) {                                                                 \
+    return fail(ctx, GK_EINVAL, "internal error");                                \
+  }
+
+extern "C" {
+
+int gk_create(const gk_grid *g, const gk_species *sp, const gk_salpha *geo, const gk_opts *o,
+              void *cuda_stream, gk_ctx **out) {
+  try {
+    return create_impl(g, sp, geo, o, cuda_stream, out);
+  } catch (const std::bad_alloc &) {
+    return GK_ENOMEM;
+  } catch (...) {
+    return GK_EINVAL;
+  }
 }
 
 int gk_destroy(gk_ctx *c) {
@@ -426,7 +466,7 @@ int gk_rhs(gk_ctx *c, const void *f, void *phi, void *rhs) {
   A.gchi = (float2 *)((char *)c->ws + c->off_gchi);
   A.chis = (float2 *)((char *)c->ws + c->off_chis);
   A.nlbuf = (float2 *)((char *)c->ws + c->off_nl);
-  A.nwork = c->P.nsp * c->P.nmu * c->P.ns * c->P.nchunk;
+  A.nwork = c->stage_nwork;
   stage_launch(c, A);
   return check_launch(c, "stage kernel");
 }
@@ -446,7 +486,7 @@ int gk_rk4_steps(gk_ctx *c, void *f, double dt, int nsteps) {
   A.gchi = (float2 *)(ws + c->off_gchi);
   A.chis = (float2 *)(ws + c->off_chis);
   A.nlbuf = (float2 *)(ws + c->off_nl);
-  A.nwork = c->P.nsp * c->P.nmu * c->P.ns * c->P.nchunk;
+  A.nwork = c->stage_nwork;
   const float h = (float)dt;
   for (int s = 0; s < nsteps; ++s) {
     if (s == 0) {  // later steps reuse the moment planes written by the previous stage 4
@@ -456,28 +496,17 @@ int gk_rk4_steps(gk_ctx *c, void *f, double dt, int nsteps) {
     }
     // classical RK4: acc = f + dt/6 k1, then += dt/3 k2, += dt/3 k3, f = acc + dt/6 k4
     if (int r = solve_phi_from_planes(c, mom, phi)) return r;
-    // kernels that do not accumulate the moment of the new state themselves are followed by gk_moment_kernel
-    auto moment_of = [&](const void *state) {
-      if (!c->host_moment) return;
-#define GK_CALL(ST) launch_moment<ST>(c, state, mom)
-      GK_BY_STORAGE(c, GK_CALL);
-#undef GK_CALL
-    };
     A.mode = 1; A.y = f; A.fn = f; A.out = ya; A.c = 0.5f * h; A.b = h / 6.f;
     stage_launch(c, A);
-    moment_of(ya);
     if (int r = solve_phi_from_planes(c, mom, phi)) return r;
     A.mode = 2; A.y = ya; A.fn = f; A.out = yb; A.c = 0.5f * h; A.b = h / 3.f;
     stage_launch(c, A);
-    moment_of(yb);
     if (int r = solve_phi_from_planes(c, mom, phi)) return r;
     A.mode = 2; A.y = yb; A.fn = f; A.out = ya; A.c = h; A.b = h / 3.f;
     stage_launch(c, A);
-    moment_of(ya);
     if (int r = solve_phi_from_planes(c, mom, phi)) return r;
     A.mode = 3; A.y = ya; A.fn = f; A.out = f; A.c = 0.f; A.b = h / 6.f;
     stage_launch(c, A);
-    moment_of(f);
     if (int r = check_launch(c, "stage kernel")) return r;
   }
   return GK_OK;
@@ -594,7 +623,7 @@ size_t gk_export_table(const gk_ctx *c, const char *which, double *out, size_t m
   } else if (w == "pad") {
     tmp = {(double)c->P.mx, (double)c->P.my, (double)c->P.rc, (double)c->P.gchi_in_smem,
            (double)c->P.jchunk, (double)c->P.nchunk, (double)c->stage_grid, (double)c->stage_smem,
-           (double)c->stage_threads, (double)c->stage_occ, (double)c->stage_ws, (double)c->stage_kind};
+           (double)c->stage_threads, (double)c->stage_cluster, (double)c->stage_nsh, (double)c->stage_kind};
     src = &tmp;
   } else return 0;
   if (out) std::memcpy(out, src->data(), std::min(maxn, src->size()) * sizeof(double));

@@ -459,14 +459,14 @@ gk_stage_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkStage
             const int e = tid + k * NT;
             if (k + 1 < EPT || e < slab) {
               const float2 out = point(modec, intc, e, ip0 + k * RS, m, pk0 + (float)(k * RS), fmf);
-              macc[k] = cadd(macc[k], out);
+              macc[k] = cadd(macc[k], as_stored<ST>(out));   // what the next stage will read back
             }
           }
         } else {
           for (int e = tid; e < slab; e += nthr) {
             const int ip = e / nky, m = e - ip * nky;
             const float2 out = point(modec, intc, e, ip, m, (float)(ip - K), (float)m);
-            if (A.mom) stage[NL ? (ip * ldx + m) : e] = out;
+            if (A.mom) stage[NL ? (ip * ldx + m) : e] = as_stored<ST>(out);
           }
           if (A.mom) {  // the same thread wrote these entries: no barrier needed
 #pragma unroll

@@ -20,44 +20,10 @@
 //                          output to the dead columns nky..2nky-1
 //   XF2 forward x pass 2   retained kx -> the bracket ring in L2 for the epilogue role
 // Twiddles come from compile-time tables in constant memory (warp-uniform indices).
-// Epilogue role: ws_epilogue_role of gk_stage_ws.cuh.
+// Epilogue role: ws_epilogue_role2 below.
 #pragma once
 
-// layout of the epilogue coefficient block (floats)
-#define GK_EB_WS 0     // [5] parallel stencil, interior class (centre: I + dissipation)
-#define GK_EB_WO 5     // [5] parallel stencil at an open chain end of this plane (ghost weights 0)
-#define GK_EB_WV 10    // [4] vpar stencil j-2, j-1, j+1, j+2 (zero padding folded in)
-#define GK_EB_WVC 14   // vpar stencil centre
-#define GK_EB_C7 15
-#define GK_EB_A2 16
-#define GK_EB_A5 17    // a5 * ky0
-#define GK_EB_A8 18
-#define GK_EB_N 20
-
 namespace gk {
-
-__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t *bar, int count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-}
-// one thread: arm the barrier with the byte count and start the bulk copy global -> shared
-__device__ __forceinline__ void bulk_load(void *dst, const void *src, uint32_t bytes, uint64_t *bar) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-               ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
-  uint32_t ok = 0;
-  while (!ok) {
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
-        "selp.u32 %0, 1, 0, p;\n"
-        "}\n" : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
-  }
-}
 
 // Twiddle tables of the two-pass transforms N = R1 R2 in constant memory (compile-time initialised; warp-uniform
 // indices, so the loads go through the constant cache and not through the shared-memory/L1 data pipe that bounds
@@ -108,17 +74,12 @@ constexpr size_t ws2_smem_bytes() {
 // kept in a small shared block (2-slot ring); every point then needs 14 operands and one packed FMA
 // per operand.  Parallel-stencil planes next to the s boundary run the same branch-free code with
 // the kx connection folded into one per-thread offset (R6) and one predicate per point
-// (open chain end: PAPER.md:350, 362; R7).
-
-// MACC: the velocity-space moment of the new state is accumulated in registers over the vpar march (one
-// float2 per point of the thread); false for slabs too large for that (the host then runs gk_moment_kernel
-// on the new state).
-// CHI_ITEM: chis_cta is the base of a scratch indexed by (species, mu, s) instead of a per-CTA ring.
-template <class ST, int NKY_, int NKX_, int NTF, int NTE, int NB, bool MACC = true, bool CHI_ITEM = false>
+// (open chain end: PAPER.md:350, 362; R7).  The velocity-space moment of the new state is accumulated
+// in registers over the vpar march (one float2 per point of the thread).
+template <class ST, int NKY_, int NKX_, int NTF, int NTE, int NB>
 __device__ __forceinline__ void ws_epilogue_role2(const GkDev &P, const GkStageArgs &A, float2 *chis_cta,
                                                   const float2 *nl_cta, float *eblk, int tid) {
   constexpr int NT = NTF + NTE;
-  constexpr bool NL = NTF > 0;   // NTF == 0: the whole CTA runs this role and term III is off
   constexpr int nky = NKY_, nkx = NKX_;
   constexpr int K = (nkx - 1) / 2, slab = nkx * nky;
   constexpr int BAR_FULL = GK_WS_BAR_FULL, BAR_FREE = GK_WS_BAR_FREE;
@@ -139,13 +100,7 @@ __device__ __forceinline__ void ws_epilogue_role2(const GkDev &P, const GkStageA
     const int al = w / (P.ns * P.nchunk);
     const int l = al % P.nmu, a = al / P.nmu;
     const long long base0 = (((long long)a * P.nv * P.nmu + l) * P.ns + i) * P.slab;
-    const float2 *chip = (CHI_ITEM ? chis_cta + (((long long)a * P.nmu + l) * P.ns + i) * (3 * slab)
-                                   : chis_cta + (it % GK_WS_CHI_RING) * 3 * slab) + et;
-    // without an FFT role the CTA builds chi and D_s chi itself; the first barrier below publishes them
-    if constexpr (!NL) {
-      build_chis(P, A, a, l, i, slab, nky, chis_cta + (it % GK_WS_CHI_RING) * 3 * slab, et, NTE);
-      bar_sync_n(BAR_FULL, NT);   // the only CTA-wide barrier of an item: warps march along vpar on their own
-    }
+    const float2 *chip = chis_cta + (it % GK_WS_CHI_RING) * 3 * slab + et;
     // per item: kappa = -(pk ksx + m kcz), hyper-viscosity hx4 (p/K)^4 + hy4 (m/(nky-1))^4
     const int mask = P.mask;
     const float ksx = P.dkx * P.sth[i], kcz = P.ky0 * P.cz[i];
@@ -163,48 +118,16 @@ __device__ __forceinline__ void ws_epilogue_role2(const GkDev &P, const GkStageA
       else if (i2 < 0) { i2 += P.ns; wrap = -1; }
       soff[q] = (i2 - i) * slab + wrap * mk * nky;
     }
-    float2 macc[MACC ? EPT : 1];
+    float2 macc[EPT];
 #pragma unroll
-    for (int k = 0; k < (MACC ? EPT : 1); ++k) macc[k] = make_float2(0.f, 0.f);
+    for (int k = 0; k < EPT; ++k) macc[k] = make_float2(0.f, 0.f);
     const int j0 = c * P.jchunk, j1 = min(P.nv, (c + 1) * P.jchunk);
     for (int j = j0; j < j1; ++j, ++u) {
-      // coefficient block: one per CTA and slab parity beside an FFT role (published by BAR_FULL), one per warp otherwise
-      float *eb = NL ? eblk + (u & 1) * GK_EB_N : eblk + (et >> 5) * GK_EB_N;
-      if constexpr (!NL) __syncwarp();
+      // coefficient block: one per slab parity, published by BAR_FULL
+      float *eb = eblk + (u & 1) * GK_EB_N;
       const bool m2 = j >= 2, m1 = j >= 1, p1 = j + 1 < P.nv, p2 = j + 2 < P.nv;
-      const float vj = P.v[j];
-      const int sg = (vj > 0.f) ? 0 : 1;
-      if (NL ? et == 0 : (et & 31) == 0) {  // slab-uniform coefficients, one thread
-        const GkSpeciesDev &Sp = P.sp[a];
-        const float mul = P.mu[l], muB = mul * P.B[i];
-        const float E = vj * vj + 2.f * muB, ED = vj * vj + muB;
-        const float fm = P.fmv[j] * P.fmm[l * P.ns + i];
-        const float cpar = Sp.vR * P.F[i] * vj;
-        const float cmir = Sp.vR * mul * P.BG[i];
-        const float cI = (mask & GK_T_I) ? -cpar * P.ds_inv : 0.f;
-        const float cDs = (mask & GK_T_DISS_S) ? -P.nu_s * fabsf(cpar) * P.ds_inv : 0.f;
-        const float c4 = (mask & GK_T_IV) ? cmir * P.dv_inv : 0.f;
-        const float cDv = (mask & GK_T_DISS_V) ? -P.nu_v * fabsf(cmir) * P.dv_inv : 0.f;
-        const int cls = lowp ? i : (i >= P.ns - 2 ? i - (P.ns - 3) + 2 : 2);
-#pragma unroll
-        for (int d = 0; d < 5; ++d) {
-          eb[GK_EB_WS + d] = cI * P.dcoef[2][sg][d] + cDs * P.discoef[2][d];
-          const int i2 = i + d - 2;
-          const bool ghost = (i2 < 0) || (i2 >= P.ns);
-          eb[GK_EB_WO + d] = ghost ? 0.f : cI * P.dcoef[cls][sg][d] + cDs * P.discoef[cls][d];
-        }
-        // D_v = (1,-8,0,8,-1)/12, delta^4_v/12 = (1,-4,6,-4,1)/12; ghosts outside the grid are zero
-        const float k1 = 1.f / 12.f, k8 = 8.f / 12.f, k4 = 4.f / 12.f;
-        eb[GK_EB_WV + 0] = m2 ? (c4 * k1 + cDv * k1) : 0.f;
-        eb[GK_EB_WV + 1] = m1 ? (-c4 * k8 - cDv * k4) : 0.f;
-        eb[GK_EB_WV + 2] = p1 ? (c4 * k8 - cDv * k4) : 0.f;
-        eb[GK_EB_WV + 3] = p2 ? (-c4 * k1 + cDv * k1) : 0.f;
-        eb[GK_EB_WVC] = cDv * 0.5f;
-        eb[GK_EB_C7] = (mask & GK_T_VII) ? -Sp.ZoverT * cpar * fm * P.ds_inv : 0.f;
-        eb[GK_EB_A2] = (mask & GK_T_II) ? Sp.ToverZ * ED : 0.f;
-        eb[GK_EB_A5] = (mask & GK_T_V) ? 0.5f * fm * (Sp.rln + (E - 1.5f) * Sp.rlt) * P.ky0 : 0.f;
-        eb[GK_EB_A8] = (mask & GK_T_VIII) ? ED * fm : 0.f;
-      }
+      const int sg = (P.v[j] > 0.f) ? 0 : 1;
+      if (et == 0) epi_coefficients(P, a, l, i, j, eb);
       const long long sb = base0 + (long long)j * jstride;
       const ST *yp = (const ST *)A.y + sb + et;
       const ST *fnp = (const ST *)A.fn + sb + et;
@@ -225,8 +148,7 @@ __device__ __forceinline__ void ws_epilogue_role2(const GkDev &P, const GkStageA
       }
       const float2 *nlr = nl_cta + (u & 1) * slab + et;
       const float2 *dsp = chip + (1 + sg) * slab;
-      if constexpr (NL) bar_sync_n(BAR_FULL + (u & 1), NT);   // also publishes eb to the role's other threads
-      else __syncwarp();
+      bar_sync_n(BAR_FULL + (u & 1), NT);   // also publishes eb to the role's other threads
       auto sweep = [&](auto modec, auto seamc) {
         constexpr int MODE = decltype(modec)::value;
         constexpr bool SEAM = decltype(seamc)::value != 0;
@@ -261,23 +183,7 @@ __device__ __forceinline__ void ws_epilogue_role2(const GkDev &P, const GkStageA
               if constexpr (MODE >= 2) ac[q] = Cv<ST>::ldcs(accp, eo);
               chi0[q] = __ldcg(chip + eo);    // written by this CTA earlier in the launch: L2, not the
               dschi[q] = __ldcg(dsp + eo);    // read-only path
-              nlv[q] = make_float2(0.f, 0.f);
-              if constexpr (NL) nlv[q] = __ldcg(nlr + eo);
-            }
-          }
-          if constexpr (!NL) {  // no FFT role: shared memory is unused, L1 is large: next batch's operands -> L1
-#pragma unroll
-            for (int q = 0; q < NB; ++q) {
-              const int k = k0 + NB + q, eo = k * NTE;
-              if (k < EPT && (k + 1 < EPT || et + eo < slab)) {
-                int o0 = -2 * slab, o1 = -slab, o3 = slab, o4 = 2 * slab;
-                if constexpr (SEAM) { o0 = soff[0]; o1 = soff[1]; o3 = soff[2]; o4 = soff[3]; }
-                auto pf = [](const void *ptr) { asm volatile("prefetch.global.L1 [%0];" ::"l"(ptr)); };
-                pf(yp + eo); pf(yp + eo + o0); pf(yp + eo + o1); pf(yp + eo + o3); pf(yp + eo + o4);
-                pf(yp + eo + ov0); pf(yp + eo + ov1); pf(yp + eo + ov3); pf(yp + eo + ov4);
-                if constexpr (MODE == 2) pf(fnp + eo);
-                if constexpr (MODE >= 2) pf(accp + eo);
-              }
+              nlv[q] = __ldcg(nlr + eo);
             }
           }
           asm volatile("" ::: "memory");      // coefficient loads stay behind the operand loads
@@ -308,7 +214,7 @@ __device__ __forceinline__ void ws_epilogue_role2(const GkDev &P, const GkStageA
               // -i a z = a (z.y, -z.x)
               r = gkfft::caxpy(we.x * kap, make_float2(f0[q].y, -f0[q].x), r);
               r = gkfft::caxpy(we.y * fmf + we.z * kap, make_float2(chi0[q].y, -chi0[q].x), r);
-              if constexpr (NL) r = gkfft::caxpy(scale, nlv[q], r);
+              r = gkfft::caxpy(scale, nlv[q], r);
               float2 out;
               if constexpr (MODE == 0) {
                 out = r;
@@ -322,7 +228,7 @@ __device__ __forceinline__ void ws_epilogue_role2(const GkDev &P, const GkStageA
                 out = gkfft::caxpy(A.b, r, ac[q]);
               }
               Cv<ST>::stcs(outp, eo, out);
-              if constexpr (MACC) macc[k] = cadd(macc[k], out);
+              macc[k] = cadd(macc[k], as_stored<ST>(out));   // what the next stage will read back
             }
           }
           asm volatile("" ::: "memory");      // the next batch's loads stay below this one's arithmetic
@@ -338,15 +244,15 @@ __device__ __forceinline__ void ws_epilogue_role2(const GkDev &P, const GkStageA
         case 2: by_plane(gkfft::IC<2>{}); break;
         default: by_plane(gkfft::IC<3>{}); break;
       }
-      if constexpr (NL) bar_arrive_n(BAR_FREE + (u & 1), NT);
+      bar_arrive_n(BAR_FREE + (u & 1), NT);
     }
-    if (MACC && A.mom) {
+    if (A.mom) {
       // moment plane of this item: Z n 2 pi w_v B_i w_mu J0 sum_j f   (a1 of the next stage)
       const float momw = P.sp[a].momfac * P.wmu[l] * P.B[i];
       const float *j0p = P.J0 + (((long long)a * P.nmu + l) * P.ns + i) * P.slab;
       float2 *dst = A.mom + (((long long)a * P.nmu + l) * P.nchunk + c) * P.nphi + (long long)i * P.slab;
 #pragma unroll
-      for (int k = 0; k < (MACC ? EPT : 1); ++k) {
+      for (int k = 0; k < EPT; ++k) {
         const int e = et + k * NTE;
         if (e < slab) dst[e] = gkfft::cscale(momw * __ldg(&j0p[e]), macc[k]);
       }
@@ -371,7 +277,10 @@ gk_stage_ws2_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkS
   constexpr int NC = 2 * NKY_;   // x-transformed columns: P(0..nky-1), Q(0..nky-1); Q(0) is never used
   constexpr int H = MX_ / 2;     // row pairs (p, p + H) of the forward transform
   static_assert(NTF % 128 == 0 && NTE % 128 == 0, "roles are whole warpgroups (setmaxnreg)");
-  static_assert(RF == 0 || (NTF * RF + NTE * RE <= 65536 && RF % 8 == 0 && RE % 8 == 0), "register split");
+  // setmaxnreg moves registers inside the pool the CTA was LAUNCHED with (threads x registers per thread at
+  // launch, itself limited by 16 K registers per SM sub-partition): a split that needs more never completes
+  constexpr int WPS = ((NTF + NTE) / 32 + 3) / 4, RL = (16384 / (WPS * 32)) / 8 * 8;
+  static_assert(RF == 0 || (RF % 8 == 0 && RE % 8 == 0 && NTF * RF + NTE * RE <= (NTF + NTE) * (RL < 255 ? RL : 255)), "register split");
   static_assert(RX2 > 1 && RY2 > 1 && RX2 % 2 == 0 && RY2 % 2 == 0 && RX1 % 2 == 0 && RY1 % 2 == 0, "two-pass even radices");
   static_assert(H % RX1 == 0, "a forward-x item lies in one half of the row pairs");
   static_assert(2 * NKY_ <= MY_ - NKY_ + 1, "dead columns hold the forward-x exchange");
@@ -387,7 +296,7 @@ gk_stage_ws2_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkS
   ST *stg = (ST *)sp;            // the slab being transformed, landed by the bulk copy
   uint64_t *mbar = (uint64_t *)((unsigned char *)stg + slab * sizeof(ST));
   float *eblk = (float *)(mbar + 2);  // 16-byte aligned: slab-uniform epilogue coefficients, 2 slots
-  if (tid == 0) mbar_init(mbar, 1);
+  if (tid == 0) { mbar_init(mbar, 1); mbar_init_fence(); }
   __syncthreads();
 
   if (tid < NTF) {
@@ -685,17 +594,6 @@ gk_stage_ws2_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkS
     if constexpr (RE > 0) asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(RE));
     ws_epilogue_role2<ST, NKY_, NKX_, NTF, NTE, NB>(P, A, chis_cta, nl_cta, eblk, tid);
   }
-}
-
-// Term III switched off: every thread of the CTA runs the lean epilogue (a streaming stencil + RK update);
-// OCC CTAs per SM, no FFT role, no dynamic shared memory.
-template <class ST, int NKY_, int NKX_, int NT, int NB, int OCC>
-__global__ void __launch_bounds__(NT, OCC)
-gk_stage_lin_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkStageArgs A) {
-  __shared__ __align__(16) float eblk[(NT / 32) * GK_EB_N];
-  constexpr int slab = NKX_ * NKY_;
-  float2 *chis_cta = A.chis + (long long)blockIdx.x * (GK_WS_CHI_RING * 3 * slab);
-  ws_epilogue_role2<ST, NKY_, NKX_, 0, NT, NB>(P, A, chis_cta, nullptr, eblk, threadIdx.x);
 }
 
 }  // namespace gk

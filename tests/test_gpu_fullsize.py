@@ -130,7 +130,7 @@ def test_repeated_runs_are_bit_identical(n, linear):
 SPECIALISED = {
     "cfg2_plane": (dict(nkx=85, nky=16, ky0=0.07, ikxspace=5), 2),
     "cfg3_plane": (dict(nkx=85, nky=32, ky0=0.035, ikxspace=5), 2),
-    "cfg5_plane": (dict(nkx=127, nky=64, ky0=0.0175, ikxspace=5), 4),
+    "cfg5_plane": (dict(nkx=127, nky=64, ky0=0.0175, ikxspace=5), 5),
 }
 
 
