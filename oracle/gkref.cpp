@@ -610,6 +610,153 @@ void gkref_spectra(const gkref *h, const double *phi_in, double *kx_spec, double
       }
 }
 
+// ---------------------------------------------------------------------------------------
+// CFL estimate of the time step ("estimate_timestep": "the minimum of (i) the
+// nonlinear CFL from the maximum real-space ExB velocity gradient, (ii) a von Neumann stability analysis
+// of the streaming and trapping stencils, and (iii) for kinetic electrons, a field CFL based on the
+// electrostatic Alfven frequency").  The paper prints no formula for (i) and (ii) and a dimensionally
+// garbled one for (iii); readings R21-R23 of DESIGN.md:
+//
+//  every bound is the LARGEST step for which classical RK4 is stable on the model problem, no safety
+//  factor (the caller applies one).  RK4: R(z) = 1 + z + z^2/2 + z^3/6 + z^4/24; on the imaginary axis
+//  |R(iy)| <= 1  <=>  |y| <= 2 sqrt 2.
+//
+//  R21 (i)   term III advects f with v_E = (1/2)(-d_y chi, d_x chi); a uniform velocity u acts on the
+//            retained spectrum with eigenvalues i(u_x kx + u_y ky), so
+//              lambda_NL = max over (a, l, i) and the points (x, y) of the padded real-space grid of
+//                          (1/2) ( |d_y chi| kx_max + |d_x chi| ky_max ),   dt_NL = 2 sqrt2 / lambda_NL.
+//            chi = J0_a phi with the ky = 0 column Hermitian-averaged exactly as in the bracket (R15);
+//            the real-space grid is the bracket's (pad_mx x pad_my).
+//  R22 (ii)  frozen-coefficient von Neumann analysis of terms I + IV with their dissipation on the interior
+//            stencils: symbols sigma(t) = (8 sin t - sin 2t)/6 of the centred 4th-order first derivative
+//            and d(t) = (2 - 2 cos t)^2 / 12 of delta^4/12,
+//              z(t, t') = c_s [ -i sigma(t) - nu_s d(t) ] + c_v [ +i sigma(t') - nu_v d(t') ],
+//              c_s = max_{a,j,i} |v_R v_j F_i| / ds,   c_v = max_{a,l,i} |v_R mu_l B_i G_i| / dv,
+//            dt_lin = min over the 64 x 64 angles t, t' = 2 pi k/64 of the first exit of the ray {tau z}
+//            from the RK4 stability region (located by 4096 uniform steps to 4/|z|, then bisection).
+//  R23 (iii) kinetic electrons: the cold-fluid response of every species to the parallel electric field
+//            closes with the polarisation A = sum_a Z_a^2 n_a (1 - Gamma0_a)/T_a into the electrostatic
+//            shear-Alfven (omega_H) oscillation
+//              omega_H^2(i,p,m) = sum_a (v_R,a F_i k_s)^2 Z_a^2 n_a <v_par^2> / (T_a A(i,p,m)),
+//            <v_par^2> = int v_par^2 F_M d^3v = 1/2, k_s = max_t sigma(t) / ds = 1.372 / ds the largest
+//            parallel wavenumber the stencil represents;  dt_field = 2 sqrt2 / max_{(i,p,m) != zonal (0,0)} omega_H.
+//            (PAPER.md:356 prints "omega ~ k_perp sqrt(me/mi) v_th,i/(q ds B)", the reciprocal of this
+//            dependence on k_perp, mass ratio and B: taken as a garbled statement of the same mode, whose
+//            frequency the operator's eigen-solve shows to scale as 1/k_perp, tests/test_oracle_cfl.py.)
+//            +infinity with adiabatic electrons.
+//  out[0] = min(out[1], out[2], out[3]); out[1] = dt_NL (+inf if phi = 0 or term III is off),
+//  out[2] = dt_lin, out[3] = dt_field.
+// ---------------------------------------------------------------------------------------
+static double rk4_amp2(std::complex<double> z) {
+  std::complex<double> R = 1.0 + z * (1.0 + z * (0.5 + z * (1.0 / 6.0 + z / 24.0)));
+  return std::norm(R);
+}
+// first exit of the ray {tau z, tau > 0} from |R| <= 1
+static double rk4_ray_limit(std::complex<double> z) {
+  const double az = std::abs(z);
+  if (az == 0.0) return HUGE_VAL;
+  const int NSTEP = 4096;
+  const double tmax = 4.0 / az;
+  double lo = 0.0, hi = -1.0;
+  for (int k = 1; k <= NSTEP; ++k) {
+    double t = tmax * k / NSTEP;
+    if (rk4_amp2(t * z) > 1.0 + 1e-13) { hi = t; break; }
+    lo = t;
+  }
+  if (hi < 0.0) return tmax;
+  for (int it = 0; it < 80; ++it) {
+    double mid = 0.5 * (lo + hi);
+    if (rk4_amp2(mid * z) > 1.0 + 1e-13) hi = mid; else lo = mid;
+  }
+  return lo;
+}
+
+void gkref_estimate_dt(const gkref *h, const double *phi_in, double *out) {
+  const cplx *phi = (const cplx *)phi_in;
+  const cplx I1(0.0, 1.0);
+  const double lim = 2.0 * std::sqrt(2.0);
+  // ---- (i) nonlinear ----
+  double lamnl = 0.0;
+  if (h->on(GKREF_T_III)) {
+    const int nkx = h->nkx, nky = h->nky, K = h->K, M = nky - 1;
+    int mx = h->o.pad_mx > 0 ? h->o.pad_mx : smooth7(3 * K + 1);
+    int my = h->o.pad_my > 0 ? h->o.pad_my : smooth7(3 * M + 1);
+    for (int a = 0; a < h->nsp; ++a)
+      for (int l = 0; l < h->nmu; ++l)
+        for (int i = 0; i < h->ns; ++i) {
+          std::vector<cplx> gx((size_t)mx * my, 0.0), gy((size_t)mx * my, 0.0);
+          for (int ip = 0; ip < nkx; ++ip)
+            for (int m = 0; m <= M; ++m) {
+              cplx c = h->J0[h->jidx(a, l, i, ip, m)] * phi[h->pidx(i, ip, m)];
+              int p = ip - K;
+              if (m == 0) {  // Hermitian average of the ky = 0 column (R15)
+                int iq = nkx - 1 - ip;
+                c = 0.5 * (c + std::conj(h->J0[h->jidx(a, l, i, iq, 0)] * phi[h->pidx(i, iq, 0)]));
+              }
+              int x = (p % mx + mx) % mx;
+              gx[(size_t)x * my + m] = I1 * (p * h->dkx) * c;
+              gy[(size_t)x * my + m] = I1 * (m * h->g.ky0) * c;
+              if (m > 0) {  // g(-p, -m) = conj g(p, m)
+                int x2 = ((-p) % mx + mx) % mx, y2 = my - m;
+                gx[(size_t)x2 * my + y2] = I1 * (-p * h->dkx) * std::conj(c);
+                gy[(size_t)x2 * my + y2] = I1 * (-m * h->g.ky0) * std::conj(c);
+              }
+            }
+          fft2d(gx, mx, my, +1);
+          fft2d(gy, mx, my, +1);
+          for (size_t n = 0; n < gx.size(); ++n) {
+            double lam = 0.5 * (std::fabs(gy[n].real()) * h->kxmax + std::fabs(gx[n].real()) * h->kymax);
+            lamnl = std::max(lamnl, lam);
+          }
+        }
+  }
+  out[1] = lamnl > 0.0 ? lim / lamnl : HUGE_VAL;
+  // ---- (ii) von Neumann, streaming + trapping ----
+  double cs = 0.0, cv = 0.0;
+  for (int a = 0; a < h->nsp; ++a)
+    for (int i = 0; i < h->ns; ++i) {
+      for (int j = 0; j < h->nv; ++j) cs = std::max(cs, std::fabs(h->vR[a] * h->v[j] * h->F[i]) / h->ds);
+      for (int l = 0; l < h->nmu; ++l) cv = std::max(cv, std::fabs(h->vR[a] * h->mu[l] * h->BG[i]) / h->dv);
+    }
+  if (!h->on(GKREF_T_I)) cs = 0.0;
+  if (!h->on(GKREF_T_IV)) cv = 0.0;
+  const double nus = h->on(GKREF_T_DISS_S) ? h->o.disp_par : 0.0, nuv = h->on(GKREF_T_DISS_V) ? h->o.disp_vp : 0.0;
+  const int NA = 64;
+  double dtlin = HUGE_VAL;
+  for (int k1 = 0; k1 < NA; ++k1)
+    for (int k2 = 0; k2 < NA; ++k2) {
+      double t1 = 2.0 * PI * k1 / NA, t2 = 2.0 * PI * k2 / NA;
+      double s1 = (8.0 * std::sin(t1) - std::sin(2.0 * t1)) / 6.0, d1 = std::pow(2.0 - 2.0 * std::cos(t1), 2) / 12.0;
+      double s2 = (8.0 * std::sin(t2) - std::sin(2.0 * t2)) / 6.0, d2 = std::pow(2.0 - 2.0 * std::cos(t2), 2) / 12.0;
+      cplx z = cs * cplx(-nus * d1, -s1) + cv * cplx(-nuv * d2, s2);
+      dtlin = std::min(dtlin, rk4_ray_limit(z));
+    }
+  out[2] = dtlin;
+  // ---- (iii) field CFL, kinetic electrons only ----
+  out[3] = HUGE_VAL;
+  if (!h->o.adiabatic_electrons && h->on(GKREF_T_I) && h->on(GKREF_T_VII)) {
+    double smax = 0.0;  // max_t sigma(t), located on a fine grid (the maximum is flat: 1.3722)
+    for (int k = 0; k <= 100000; ++k) {
+      double t = PI * k / 100000.0;
+      smax = std::max(smax, (8.0 * std::sin(t) - std::sin(2.0 * t)) / 6.0);
+    }
+    double om2 = 0.0;
+    for (int i = 0; i < h->ns; ++i)
+      for (int ip = 0; ip < h->nkx; ++ip)
+        for (int m = 0; m < h->nky; ++m) {
+          if (ip == h->K && m == 0) continue;
+          double num = 0.0;
+          for (int a = 0; a < h->nsp; ++a) {
+            double c = h->vR[a] * h->F[i] * smax / h->ds;
+            num += c * c * h->sp[a].Z * h->sp[a].Z * h->sp[a].dens * 0.5 / h->sp[a].temp;
+          }
+          om2 = std::max(om2, num / h->Apol[h->pidx(i, ip, m)]);
+        }
+    if (om2 > 0.0) out[3] = lim / std::sqrt(om2);
+  }
+  out[0] = std::min(out[1], std::min(out[2], out[3]));
+}
+
 void gkref_bracket_slab(const gkref *h, const double *chi, const double *fs, int method, int mx,
                         int my, double *out) {
   h->bracket((const cplx *)chi, (const cplx *)fs, method, mx, my, (cplx *)out);

@@ -77,6 +77,11 @@ void gkref_fluxes(const gkref *, const double *f, const double *phi, double *out
  * kx_spec[nkx], ky_spec[nky] */
 void gkref_spectra(const gkref *, const double *phi, double *kx_spec, double *ky_spec);
 
+/* CFL estimate of the largest stable RK4 step (readings R21-R23, see gkref.cpp):
+ * out[0] = min of out[1] = nonlinear (ExB) bound for this phi, out[2] = von Neumann bound of the streaming and
+ * trapping stencils, out[3] = field (omega_H) bound with kinetic electrons (+inf otherwise).  No safety factor. */
+void gkref_estimate_dt(const gkref *, const double *phi, double *out4);
+
 /* bracket of two spectral slabs (nkx*nky complex each): 0.5*sum (k'x k''y - k'y k''x) chi f */
 void gkref_bracket_slab(const gkref *, const double *chi, const double *fs, int method, int mx,
                         int my, double *out);

@@ -73,6 +73,7 @@ def _load():
         lib.gkref_rk4_step.argtypes = [C.c_void_p, dp, C.c_double]
         lib.gkref_fluxes.argtypes = [C.c_void_p, dp, dp, dp]
         lib.gkref_spectra.argtypes = [C.c_void_p, dp, dp, dp]
+        lib.gkref_estimate_dt.argtypes = [C.c_void_p, dp, dp]
         lib.gkref_bracket_slab.argtypes = [C.c_void_p, dp, dp, C.c_int, C.c_int, C.c_int, dp]
         lib.gkref_table.restype = C.c_size_t
         lib.gkref_table.argtypes = [C.c_void_p, C.c_char_p, dp]
@@ -160,6 +161,13 @@ class GkRef:
         kxs, kys = np.empty(self.shape[4], np.float64), np.empty(self.shape[5], np.float64)
         _load().gkref_spectra(self._h, _dp(phi), _dp(kxs), _dp(kys))
         return kxs, kys
+
+    def estimate_dt(self, phi):
+        """(dt, dt_nl, dt_lin, dt_field): largest RK4-stable steps (R21-R23), no safety factor."""
+        phi = self._c128(phi, self.phi_shape)
+        out = np.empty(4, np.float64)
+        _load().gkref_estimate_dt(self._h, _dp(phi), _dp(out))
+        return out
 
     def bracket_slab(self, chi, fs, method=0, mx=0, my=0):
         chi = self._c128(chi, self.shape[4:])
