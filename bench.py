@@ -43,12 +43,61 @@ def _peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-def _traffic(workload):
+def _ncu_record(workload):
+    """Per-launch counters of the stage kernel from the committed ncu capture (profiles/stage_traffic.json):
+    {"dram_gb": ..., "l1_wavefronts": ...} or None if this workload was not captured."""
     p = os.path.join(ROOT, "profiles", "stage_traffic.json")
     if os.path.exists(p):
         with open(p) as fh:
             return json.load(fh).get(workload)
     return None
+
+
+SM_COUNT, FP32_LANES, SM_MAX_MHZ = 148, 128, 1965.0      # B200 (B200_PROFILING.md)
+
+
+def fp32_flops_per_point(grid, plan, nonlinear):
+    """fp32 flop model of one stage per grid point: 5 n log2 n per complex
+    length-n transform; a real 2-D transform = x transforms on the nky non-zero columns + half-cost (c2r / r2c) y
+    transforms on the mx rows; three real 2-D transforms per slab (d_x f, d_y f inverse, bracket forward) plus the two
+    of grad(chi) amortised over vpar, 3 flops per real-space point for the product, about 100 for the linear terms
+    and the RK update."""
+    lin = 100.0
+    if not nonlinear:
+        return lin
+    mx, my, nkx, nky, nv = plan["mx"], plan["my"], grid["nkx"], grid["nky"], grid["nvpar"]
+    t2d = nky * 5.0 * mx * np.log2(mx) + mx * 0.5 * 5.0 * my * np.log2(my)
+    return ((3.0 + 2.0 / nv) * t2d + 3.0 * mx * my) / (nkx * nky) + lin
+
+
+def stage_rooflines(cfg, plan, npts, storage, stage_avg_ms, sm_mhz, nonlinear):
+    """The three ceilings of one stage-kernel launch: HBM (algorithmic bytes / measured copy bandwidth), fp32 FMA
+    pipes (flop model / 148 SMs x 128 lanes x 2 x clock) and the L1 / shared-memory data pipe (wavefronts counted by
+    ncu for this kernel / one 128-byte wavefront per SM per clock)."""
+    peak, peak_src = _peaks()
+    bpp = ALG_BYTES_PER_POINT_STAGE[storage]
+    t = stage_avg_ms * 1e-3
+    achieved = bpp * npts / t / 1e9
+    key = cfg["name"] + ("" if nonlinear else "+linear") + ("" if storage == 0 else "+half")
+    rec = _ncu_record(key) or {}
+    clock = (sm_mhz or SM_MAX_MHZ) * 1e6
+    fpp = fp32_flops_per_point(cfg["grid"], plan, nonlinear)
+    fp32_peak = SM_COUNT * FP32_LANES * 2 * SM_MAX_MHZ * 1e6 / 1e12
+    fp32 = fpp * npts / t / 1e12
+    out = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+           "traffic": rec.get("dram_gb"),
+           "traffic_unit": "GB of DRAM read+write per stage-kernel launch (ncu --set full, profiles/)",
+           "peak_source": peak_src, "avg_launch_ms": stage_avg_ms, "alg_bytes_per_point": bpp,
+           "fp32": {"bound": "alu", "achieved": fp32, "peak": fp32_peak, "unit": "TFLOP/s", "frac": fp32 / fp32_peak,
+                    "flops_per_point": fpp, "peak_source": "148 SM x 128 lanes x 2 x 1.965 GHz (B200_PROFILING.md)"}}
+    wf = rec.get("l1_wavefronts")
+    if wf:
+        cyc = t * clock
+        out["l1_shared_pipe"] = {"bound": "l1", "achieved": wf / cyc / SM_COUNT, "peak": 1.0,
+                                 "unit": "128-byte wavefronts per SM per clock", "frac": wf / cyc / SM_COUNT,
+                                 "wavefronts_per_launch": wf,
+                                 "source": "l1tex__data_pipe_lsu_wavefronts of the committed ncu capture / the live launch time"}
+    return out
 
 
 class ClockSampler:
@@ -252,14 +301,15 @@ def run_cufft_compare(args, cfg):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=3, help="BASELINE.json config number 1..5")
+    ap.add_argument("--config", type=int, default=5, help="BASELINE.json config number 1..5 (default: the largest, config 5 with complex64 storage)")
     ap.add_argument("--impl", default="gk", choices=["gk", "reference"])
     ap.add_argument("--storage", type=int, default=None, help="override storage (0 c64, 1 fp16, 2 bf16)")
     ap.add_argument("--linear", action="store_true", help="switch term III off (HBM-bound variant)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs)")
+    ap.add_argument("--no-secondary", action="store_true", help="skip the config-3 stage timing that follows a config-5 run")
     ap.add_argument("--compare", default=None, choices=["cufft"], help="measured comparison: term III through cuFFT, unfused")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "gk" else args.warmup
@@ -295,29 +345,39 @@ def main():
     g = GkContext(cfg, device=dev)
     f_host = gkinputs.initial_f(cfg, np.complex64)
     fd = g.to_state(f_host)
+    del f_host
     npts = int(np.prod(g.shape))
     dt = cfg["dt"]
     storage = g.storage
+    nl = bool(cfg["opts"]["nonlinear"])
+
+    def timed_steps(ctx, state, steps):
+        """EXACTLY `steps` RK4 steps in one timed region (CUDA events on the context stream = torch's current
+        stream); an event after every step gives the per-step times (median of >= 5 repetitions)."""
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]
+        ctx.gk_set_profiling(True)
+        ctx.gk_stage_kernel_time(reset=True)
+        l0 = ctx.gk_launch_count()
+        ev[0].record()
+        for k in range(steps):
+            ctx.gk_rk4_steps(state, dt, 1)
+            ev[k + 1].record()
+        barrier()
+        total = ev[0].elapsed_time(ev[-1])
+        per = [ev[k].elapsed_time(ev[k + 1]) for k in range(steps)]
+        n_launch = ctx.gk_launch_count() - l0
+        stage_ms, stage_n = ctx.gk_stage_kernel_time(reset=True)
+        ctx.gk_set_profiling(False)
+        return total, per, n_launch, stage_ms, stage_n
 
     # ---- device-resident throughput ----
     g.gk_rk4_steps(fd, dt, args.warmup)
     barrier()
     sampler = ClockSampler(local_rank)
     sampler.start()
-    g.gk_set_profiling(True)
-    g.gk_stage_kernel_time(reset=True)
-    l0 = g.gk_launch_count()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     sampler.mark()
-    e0.record()
-    g.gk_rk4_steps(fd, dt, args.steps)
-    e1.record()
-    barrier()
+    ms, per_step, launches, stage_ms, stage_n = timed_steps(g, fd, args.steps)
     sampler.mark()
-    ms = e0.elapsed_time(e1)
-    launches = g.gk_launch_count() - l0
-    stage_ms, stage_n = g.gk_stage_kernel_time(reset=True)
-    g.gk_set_profiling(False)
     clocks = sampler.stop()
     finite = bool(torch.isfinite(torch.view_as_real(fd) if storage == 0 else fd.float()).all().item())
     ms_max = max_over_ranks(ms, world, dev)
@@ -330,18 +390,20 @@ def main():
     hbuf = torch.empty(fd.shape if e2e_steps else (1,), dtype=fd.dtype).pin_memory()
     if e2e_steps:
         hbuf.copy_(fd.cpu())
-    # serial form: one C-ABI call per step on HOST buffers (H2D + 4 stages + D2H back to back on one stream)
+    # a time advance: one C-ABI call per step on HOST buffers, each step uploads its input and downloads its result
+    # (H2D + 4 stages + D2H back to back on one stream; step k+1 depends on step k, nothing overlaps)
     for _ in range(2 if e2e_steps else 0):
         g.gk_rk4_step_host(hbuf, hbuf, fd, dt)
     barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
     for _ in range(e2e_steps):
         g.gk_rk4_step_host(hbuf, hbuf, fd, dt)
     e1.record()
     barrier()
     serial_ms = max_over_ranks(e0.elapsed_time(e1), world, dev) if e2e_steps else None
-    # pipelined form: the same steps as one C-ABI batch call (upload of step k+1 and download of step k-1 overlap
-    # the compute of step k over two device buffers); every step still uploads its input and downloads its result
+    # a batch of INDEPENDENT problems (an ensemble, not a time advance) as one C-ABI call: the upload of problem k+1
+    # and the download of problem k-1 overlap the compute of problem k over two device buffers
     if e2e_steps:
         hout = torch.empty_like(hbuf).pin_memory()
         fd2 = g.empty_state()
@@ -352,41 +414,65 @@ def main():
         g.gk_rk4_batch_host([hbuf] * e2e_steps, [hout] * e2e_steps, fd, fd2, dt)
     e1.record()
     barrier()
-    e2e_ms = max_over_ranks(e0.elapsed_time(e1), world, dev)
-    e2e_value = aggregate_value(npts, e2e_steps, world, e2e_ms) if e2e_steps else None
+    batch_ms = max_over_ranks(e0.elapsed_time(e1), world, dev)
     fbytes = fd.numel() * fd.element_size()
+    plan = g.plan()
+    kernel_names = {0: "gk_stage_kernel", 2: "gk_stage_ws2_kernel", 3: "gk_stage_lin_kernel", 5: "gk_stage_ws4_kernel"}
+
+    # ---- secondary workload (rank 0, N = 1): the stage kernel of BASELINE config 3 (the round-1 headline) ----
+    secondary = None
+    if rank == 0 and world == 1 and args.config == 5 and not args.no_secondary:
+        del g, fd, hbuf
+        if e2e_steps:
+            del hout, fd2
+        torch.cuda.empty_cache()
+        cfg3 = replica_config(3, rank, None, args.linear)
+        g3 = GkContext(cfg3, device=dev)
+        f3 = g3.to_state(gkinputs.initial_f(cfg3, np.complex64))
+        g3.gk_rk4_steps(f3, cfg3["dt"], args.warmup)
+        barrier()
+        ms3, per3, _, st3, sn3 = timed_steps(g3, f3, max(5, min(args.steps, 10)))
+        n3 = int(np.prod(g3.shape))
+        p3 = g3.plan()
+        secondary = {"workload": cfg3["name"], "points": n3, "value": n3 * 4 * len(per3) / (ms3 * 1e-3), "unit": UNIT,
+                     "ms_per_step_median": float(np.median(per3)), "kernel": kernel_names[p3["kind"]],
+                     "roofline": stage_rooflines(cfg3, p3, n3, g3.storage, st3 / max(sn3, 1), clocks.get("sm_mhz"),
+                                                 bool(cfg3["opts"]["nonlinear"]))}
+        del g3, f3
+        torch.cuda.empty_cache()
 
     if rank == 0:
-        peak, peak_src = _peaks()
-        bpp = ALG_BYTES_PER_POINT_STAGE[storage]
         stage_avg_ms = stage_ms / max(stage_n, 1)
-        achieved = bpp * npts / (stage_avg_ms * 1e-3) / 1e9
-        plan = g.plan()
-        nl = bool(cfg["opts"]["nonlinear"])
+        roof = stage_rooflines(cfg, plan, npts, storage, stage_avg_ms, clocks.get("sm_mhz"), nl)
+        roof.update({"kernel": kernel_names[plan["kind"]], "launches_timed": int(stage_n),
+                     "stage_share_of_step": stage_ms / ms if ms > 0 else None})
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None,
             "dtype": {0: "f32", 1: "f32 (fp16 storage)", 2: "f32 (bf16 storage)"}[storage],
             "data": "synthetic",
-            "config": {"workload": cfg["name"], "grid": cfg["grid"], "nspecies": g.nsp, "points": npts,
+            "config": {"workload": cfg["name"], "grid": cfg["grid"], "nspecies": len(cfg["species"]), "points": npts,
                        "nonlinear": nl, "dt": dt, "padded_fft": [plan["mx"], plan["my"]],
+                       "launch": {"grid": plan["stage_grid"], "threads": plan["threads"], "cluster": plan["cluster"],
+                                  "smem": plan["stage_smem"], "vpar_chunks": plan["nchunk"]},
                        "l2": "inputs larger than L2 (state + 3 work arrays)" if npts * 8 * 4 > 126e6 * 2
                        else "working set comparable to L2; not flushed",
                        "parallelism": "replicas only (paper has no grid parallelism)", "finite": finite},
+            "step_ms": {"median": float(np.median(per_step)), "min": float(np.min(per_step)),
+                        "max": float(np.max(per_step)), "repetitions": len(per_step)},
             "clocks": clocks,
-            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": fbytes, "d2h_bytes_per_step": fbytes,
-                    "steps": e2e_steps, "call": "gk_rk4_batch_host (pinned host buffers, copies pipelined with compute)",
-                    "serial_value": aggregate_value(npts, e2e_steps, world, serial_ms) if e2e_steps else None,
-                    "serial_call": "gk_rk4_step_host"},
+            "e2e": {"value": aggregate_value(npts, e2e_steps, world, serial_ms) if e2e_steps else None, "unit": UNIT,
+                    "h2d_bytes_per_step": fbytes, "d2h_bytes_per_step": fbytes, "steps": e2e_steps,
+                    "call": "gk_rk4_step_host (pinned host buffers; a time advance: every step uploads f_n, runs 4 stages, "
+                            "downloads f_n+1, nothing overlaps)",
+                    "batch_value": aggregate_value(npts, e2e_steps, world, batch_ms) if e2e_steps else None,
+                    "batch_call": "gk_rk4_batch_host (independent problems, copies pipelined with compute)"},
             "gpu_launches": int(launches),
-            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                         "frac": achieved / peak, "traffic": _traffic(cfg["name"] + ("" if nl else "+linear") + ("" if storage == 0 else "+half")),
-                         "traffic_unit": "GB of DRAM read+write per stage-kernel launch (ncu, profiles/)", "peak_source": peak_src,
-                         "kernel": {0: "gk_stage_kernel", 2: "gk_stage_ws2_kernel", 3: "gk_stage_lin_kernel", 5: "gk_stage_ws4_kernel"}[plan["kind"]], "launches_timed": int(stage_n),
-                         "avg_launch_ms": stage_avg_ms, "alg_bytes_per_point": bpp,
-                         "stage_share_of_step": stage_ms / ms if ms > 0 else None},
+            "roofline": roof,
         }
+        if secondary:
+            line["secondary"] = secondary
         if not args.no_cpu_baseline and world == 1:
             line["cpu_baseline"] = _oracle_sample(cfg, budget_s=12.0)
         print(json.dumps(line), flush=True)

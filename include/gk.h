@@ -13,7 +13,8 @@
  *   - f, rhs and the host-call device buffers must be 16-byte aligned (slabs move by bulk copies): GK_EINVAL.
  *   - Caller owns f, phi, rhs and the workspace; the context owns only its coefficient tables.
  *   - Hot calls (field_solve, rhs, rk4_step, rk4_steps) are asynchronous on the stream given to
- *     gk_create, never synchronise and never allocate.  gk_fluxes synchronises the stream.
+ *     gk_create, never synchronise and never allocate.  The diagnostics calls (gk_fluxes, gk_fluxes_last,
+ *     gk_spectra, gk_estimate_dt, gk_rk4_steps_cfl) synchronise the stream; none allocates.
  *   - Every function returns 0 (GK_OK) or a negative error code; no exception crosses the ABI.
  *     After GK_ECUDA the context is poisoned (sticky CUDA error); text in gk_last_error().
  *   - There is no CPU fallback: without a CUDA device gk_create returns GK_ECUDA.
@@ -117,8 +118,36 @@ int gk_rk4_batch_host(gk_ctx *ctx, const void *const *f_host_in, void *const *f_
                       void *f_dev0, void *f_dev1, double dt);
 
 /* Transport fluxes per species (R18): out_host[3*a + {0,1,2}] = particle, heat,
- * parallel-momentum flux.  Synchronises the stream. */
+ * parallel-momentum flux of a caller-supplied (f, phi).  One pass over f into per-block partial sums and a
+ * fixed-order second pass (deterministic, no atomics, no allocation).  Synchronises the stream. */
 int gk_fluxes(gk_ctx *ctx, const void *f_dev, const void *phi_dev, double *out_host);
+
+/* Diagnostics folded into the time step ("computed only at block boundaries").  With
+ * diagnostics on, every RK4 step's FIRST stage launch -- which holds f_n and chi = J0 phi(f_n) in registers -- also
+ * reduces the flux triple of (f_n, phi(f_n)): no extra pass over f.  gk_fluxes_last returns the fluxes of the state
+ * at the START of the most recent step taken by gk_rk4_step(s) (same layout and normalisation as gk_fluxes;
+ * deterministic: one writer per partial, fixed-order sum).  Synchronises the stream.  GK_EINVAL if no step has run
+ * since diagnostics were switched on. */
+int gk_set_diagnostics(gk_ctx *ctx, int on);
+int gk_fluxes_last(gk_ctx *ctx, double *out_host);
+
+/* CFL estimate of the time step (PAPER.md:340 estimate_timestep; readings R21-R23).  out_host[4]:
+ *   [1] nonlinear bound 2 sqrt2 / max (1/2)(|d_y chi| kx_max + |d_x chi| ky_max), the maximum taken over the padded
+ *       real-space grad(chi) of every (species, mu, s) as built by the MOST RECENT stage launch (gk_rhs or the last
+ *       stage of gk_rk4_step(s): "one-step lag"); +inf before the first launch, for phi = 0 and with term III off;
+ *   [2] von Neumann bound of the streaming and trapping stencils with their dissipation (create-time);
+ *   [3] field (omega_H) bound with kinetic electrons, +inf with adiabatic electrons (create-time);
+ *   [0] the minimum of the three.
+ * Each is the largest step for which classical RK4 is stable on the model problem; no safety factor is applied.
+ * Synchronises the stream (reads one word back). */
+int gk_estimate_dt(gk_ctx *ctx, double *out_host);
+
+/* CFL-adaptive stepping ("optional CFL-adaptive mode ... updated with one-step lag; the initial step
+ * uses a conservative linear-only estimate"): nsteps RK4 steps, step k with dt_k = min(safety * gk_estimate_dt()[0],
+ * dt_max) evaluated just before the step (dt_max <= 0: no cap).  dt_used_host (nsteps doubles) and t_advanced_host
+ * (one double) may be NULL.  Synchronises once per step. */
+int gk_rk4_steps_cfl(gk_ctx *ctx, void *f_dev, int nsteps, double safety, double dt_max, double *dt_used_host,
+                     double *t_advanced_host);
 
 /* Spectra of the potential (ky_spec = sum_{s,kx} |phi|^2, kx_spec = sum_{s,ky} |phi|^2, with the
  * Parseval factor P_ky (1 at ky = 0, 2 otherwise) and the weight Delta s = 1/ns applied; R20):
@@ -132,14 +161,6 @@ int gk_spectra(gk_ctx *ctx, const void *phi_dev, double *kx_spec_host, double *k
  * "vpar","mu","wmu","kx","ky","B","F","BG","J0","Gamma0","FM","den","zonal","pad".  Returns the
  * number of doubles (also when host_out is NULL), 0 for an unknown name. */
 size_t gk_export_table(const gk_ctx *ctx, const char *which, double *host_out, size_t max_doubles);
-
-/* Number of kernel launches issued through this context so far (bench.py's gpu_launches). */
-long long gk_launch_count(const gk_ctx *ctx);
-/* CUDA-event time (ms) spent in the stage kernel since the last call with reset!=0, and the number
- * of stage-kernel launches in that interval; events are recorded on the context stream only while
- * profiling is enabled with gk_set_profiling(ctx, 1).  Synchronises the stream. */
-int gk_set_profiling(gk_ctx *ctx, int on);
-int gk_stage_kernel_time(gk_ctx *ctx, double *ms_total, long long *launches, int reset);
 
 const char *gk_last_error(const gk_ctx *ctx); /* never NULL; "" if no error */
 const char *gk_version(void);

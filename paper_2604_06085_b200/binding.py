@@ -50,9 +50,12 @@ def lib_path() -> str:
 
 
 def exported_symbols() -> list[str]:
-    """Names declared in include/gk.h (functions)."""
-    with open(os.path.join(_build.INCLUDE, "gk.h")) as fh:
-        src = fh.read()
+    """Names declared in include/*.h (functions)."""
+    src = ""
+    for name in sorted(os.listdir(_build.INCLUDE)):
+        if name.endswith(".h"):
+            with open(os.path.join(_build.INCLUDE, name)) as fh:
+                src += fh.read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
     return sorted(set(re.findall(r"\b(gk_[a-z0-9_]+)\s*\(", src)))
 
@@ -87,6 +90,10 @@ def load_library(build_if_missing: bool = True):
     lib.gk_rk4_step_host.argtypes = [vp, vp, vp, vp, C.c_double]
     lib.gk_rk4_batch_host.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.c_int, vp, vp, C.c_double]
     lib.gk_spectra.argtypes = [vp, vp, dp, dp]
+    lib.gk_set_diagnostics.argtypes = [vp, C.c_int]
+    lib.gk_fluxes_last.argtypes = [vp, dp]
+    lib.gk_estimate_dt.argtypes = [vp, dp]
+    lib.gk_rk4_steps_cfl.argtypes = [vp, vp, C.c_int, C.c_double, C.c_double, dp, dp]
     lib.gk_export_table.restype = C.c_size_t
     lib.gk_export_table.argtypes = [vp, C.c_char_p, dp, C.c_size_t]
     lib.gk_launch_count.restype = C.c_longlong
@@ -254,6 +261,33 @@ class GkContext:
         self._check(self.lib.gk_fluxes(self._h, C.c_void_p(f.data_ptr()), C.c_void_p(phi.data_ptr()),
                                        out.ctypes.data_as(C.POINTER(C.c_double))))
         return out
+
+    def gk_set_diagnostics(self, on: bool):
+        self._check(self.lib.gk_set_diagnostics(self._h, int(bool(on))))
+
+    def gk_fluxes_last(self):
+        """Fluxes of the state at the start of the most recent step (diagnostics on)."""
+        import numpy as np
+        out = np.zeros((self.nsp, 3), np.float64)
+        self._check(self.lib.gk_fluxes_last(self._h, out.ctypes.data_as(C.POINTER(C.c_double))))
+        return out
+
+    def gk_estimate_dt(self):
+        """(dt, dt_nl, dt_lin, dt_field); the nonlinear bound is that of the most recent stage launch."""
+        import numpy as np
+        out = np.zeros(4, np.float64)
+        self._check(self.lib.gk_estimate_dt(self._h, out.ctypes.data_as(C.POINTER(C.c_double))))
+        return out
+
+    def gk_rk4_steps_cfl(self, f, nsteps, safety, dt_max=0.0):
+        """CFL-adaptive steps; returns (dt of every step, time advanced)."""
+        import numpy as np
+        self._chk_state(f, "f")
+        dts = np.zeros(max(int(nsteps), 1), np.float64)
+        t = C.c_double()
+        self._check(self.lib.gk_rk4_steps_cfl(self._h, C.c_void_p(f.data_ptr()), int(nsteps), float(safety), float(dt_max),
+                                              dts.ctypes.data_as(C.POINTER(C.c_double)), C.byref(t)))
+        return dts[:int(nsteps)], t.value
 
     def gk_spectra(self, phi):
         """(kx_spec[nkx], ky_spec[nky]) of |phi|^2 (PAPER.md:113, 390)."""

@@ -27,6 +27,7 @@ struct GkDev {
   int gchi_in_smem;    // 1: real-space grad(chi) lives in shared memory, 0: per-CTA global scratch
   float ds_inv, dv_inv;
   float dkx, ky0;      // kx_p = p*dkx, ky_m = m*ky0
+  float kxmax, kymax;  // K*dkx, (nky-1)*ky0: largest retained wavenumbers (CFL estimate, R21)
   float invK, invM;    // 1/K, 1/(nky-1) (0 if degenerate)
   float hyp_x, hyp_y;  // nu_x, nu_y of the hyper-viscosity (0 if masked off)
   float nu_s, nu_v;
@@ -67,4 +68,8 @@ struct GkStageArgs {
   int mode;          // 0: out = k; 1: acc = y + b k, out = y + c k; 2: acc += b k, out = fn + c k;
                      // 3: out = acc + b k
   int nwork;         // work items = nsp*nmu*ns*nchunk
+  // diagnostics folded into the launch (nullptr: off)
+  unsigned int *gmax;  // CFL (R21): atomicMax of the bits of max(|d_y chi| kx_max + |d_x chi| ky_max) over the real-space
+                     // grad(chi) this launch builds (non-negative floats order like unsigned integers)
+  double *fluxp;     // flux partial sums [cta][warp][species][3] of the state `y` (mode 1 only)
 };

@@ -43,10 +43,12 @@ __global__ void __launch_bounds__(256) gk_moment_kernel(const __grid_constant__ 
 
 // a2. phi = (sum of planes) / denominator.  For adiabatic electrons the ky=0 column receives the
 // plain division here and the flux-surface-average correction in gk_zonal_kernel (R10).
+// Also clears the CFL maximum that the stage launch following this field solve accumulates (GmaxAcc).
 __global__ void __launch_bounds__(256) gk_phi_kernel(const __grid_constant__ GkDev P,
                                                      const float2 *__restrict__ mom,
-                                                     float2 *__restrict__ phi) {
+                                                     float2 *__restrict__ phi, unsigned int *gmax) {
   const long long e = (long long)blockIdx.x * 256 + threadIdx.x;
+  if (e == 0 && gmax) *gmax = 0u;
   if (e >= P.nphi) return;
   float2 acc = make_float2(0.f, 0.f);
   for (int q = 0; q < P.nparts; ++q) acc = cadd(acc, __ldg(&mom[(long long)q * P.nphi + e]));
@@ -77,12 +79,13 @@ __global__ void __launch_bounds__(32) gk_zonal_kernel(const __grid_constant__ Gk
 }
 
 // =================================================================================================
-// Fluxes (R18).  out[3*a+q] accumulated with double atomics.
+// Fluxes (R18) of a caller-supplied (f, phi): per-block partial sums
+// part[(blockIdx.x * nsp + a) * 3 + q], summed in a fixed order by gk_flux_sum_kernel (no atomics).
 // =================================================================================================
 template <class ST>
 __global__ void __launch_bounds__(256) gk_flux_kernel(const __grid_constant__ GkDev P,
                                                       const void *__restrict__ f,
-                                                      const float2 *__restrict__ phi, double *out) {
+                                                      const float2 *__restrict__ phi, double *part) {
   const long long per_sp = P.ntot / P.nsp;
   double acc[3] = {0, 0, 0};
   const int a = blockIdx.y;
@@ -115,8 +118,20 @@ __global__ void __launch_bounds__(256) gk_flux_kernel(const __grid_constant__ Gk
   if (threadIdx.x < 3) {
     double v = 0;
     for (int w = 0; w < 8; ++w) v += red[threadIdx.x][w];
-    atomicAdd(&out[3 * a + threadIdx.x], v);
+    part[((size_t)blockIdx.x * P.nsp + a) * 3 + threadIdx.x] = v;
   }
+}
+
+// out[3 a + q] = sum over the `nslots` partial records part[slot][a][q] in slot order: one thread per output,
+// deterministic.  The partials come from gk_flux_kernel (one slot per block) or from the flux diagnostics of a
+// stage-1 launch (one slot per (CTA, warp): FluxAcc in gk_common.cuh).
+__global__ void __launch_bounds__(32) gk_flux_sum_kernel(const __grid_constant__ GkDev P, const double *__restrict__ part,
+                                                         int nslots, double *__restrict__ out) {
+  const int t = threadIdx.x;
+  if (t >= 3 * P.nsp) return;
+  double acc = 0.0;
+  for (int sl = 0; sl < nslots; ++sl) acc += part[(size_t)sl * 3 * P.nsp + t];
+  out[t] = acc;
 }
 
 // Spectra of |phi|^2 (R20).  Block b < nkx sums row p = b over (s, ky) with the Parseval

@@ -2,6 +2,7 @@
 // Product path.  No CPU fallback: every entry point needs a CUDA device.
 #include <cstdio>
 #include <cstdlib>
+#include <cmath>
 #include <cstring>
 #include <new>
 #include <stdexcept>
@@ -9,6 +10,7 @@
 #include <vector>
 
 #include "../../include/gk.h"
+#include "../../include/gk_debug.h"
 #include "gk_kernels.cuh"
 #include "gk_pick.h"
 #include "gk_tables.h"
@@ -47,6 +49,7 @@ struct gk_ctx {
   size_t ws_bytes = 0;
   size_t off_mom = 0, off_phi = 0, off_gchi = 0, off_chis = 0, off_nl = 0, off_ya = 0, off_yb = 0, off_acc = 0;
   const void *stage_fn = nullptr;  // the stage-kernel instantiation chosen at create time
+  const void *stage_fn2 = nullptr; // GK_KIND_POINT: gk_chis_kernel
   int stage_nwork = 0;
   size_t need_rhs = 0, need_full = 0;
   bool mom_valid_for_f = false;  // inside gk_rk4_steps only
@@ -58,6 +61,14 @@ struct gk_ctx {
   cudaStream_t s_up = nullptr, s_down = nullptr;
   cudaEvent_t e_in[2] = {nullptr, nullptr}, e_done[2] = {nullptr, nullptr}, e_out[2] = {nullptr, nullptr};
   size_t ev_used = 0;
+  // diagnostics: one context-owned device block (allocated by gk_create, never by a hot call):
+  // [gmax | flux_out 3*nsp | spectra nkx+nky | flux partials part_slots x nsp x 3]
+  unsigned int *d_gmax = nullptr;
+  double *d_flux_out = nullptr, *d_spec = nullptr, *d_part = nullptr;
+  int part_slots = 0;
+  bool diag = false;            // gk_set_diagnostics: fluxes of f_n folded into every stage-1 launch
+  bool flux_valid = false;
+  double dt_lin = 0, dt_field = 0;   // create-time CFL bounds (R22, R23)
 };
 
 namespace {
@@ -124,6 +135,12 @@ void stage_config(const gk_ctx *c, cudaLaunchConfig_t &cfg, cudaLaunchAttribute 
 
 void launch_stage(gk_ctx *c, const GkStageArgs &A) {
   void *args[2] = {(void *)&c->P, (void *)&A};
+  if (c->stage_kind == GK_KIND_POINT) {   // tiny (kx,ky) planes: chi planes first, then one thread per grid point
+    cudaLaunchKernel(c->stage_fn2, dim3(c->P.nsp * c->P.nmu * c->P.ns), dim3(128), args, 0, c->stream);
+    cudaLaunchKernel(c->stage_fn, dim3((unsigned)((c->P.ntot + 255) / 256)), dim3(256), args, 0, c->stream);
+    c->launches += 2;
+    return;
+  }
   cudaLaunchConfig_t cfg;
   cudaLaunchAttribute attr;
   stage_config(c, cfg, attr);
@@ -131,10 +148,13 @@ void launch_stage(gk_ctx *c, const GkStageArgs &A) {
   ++c->launches;
 }
 
-template <class ST> void launch_flux(gk_ctx *c, const void *f, const float2 *phi, double *out) {
-  dim3 grid((unsigned)std::min<long long>(4096, (c->P.ntot / c->P.nsp + 255) / 256), c->P.nsp);
-  gk::gk_flux_kernel<ST><<<grid, 256, 0, c->stream>>>(c->P, f, phi, out);
-  ++c->launches;
+constexpr int kFluxBlocks = 4096;   // most blocks (per species) gk_flux_kernel is launched with
+
+template <class ST> void launch_flux(gk_ctx *c, const void *f, const float2 *phi) {
+  dim3 grid((unsigned)std::min<long long>(kFluxBlocks, (c->P.ntot / c->P.nsp + 255) / 256), c->P.nsp);
+  gk::gk_flux_kernel<ST><<<grid, 256, 0, c->stream>>>(c->P, f, phi, c->d_part);
+  gk::gk_flux_sum_kernel<<<1, 32, 0, c->stream>>>(c->P, c->d_part, (int)grid.x, c->d_flux_out);
+  c->launches += 2;
 }
 
 #ifdef GK_ONLY_C64  // developer builds (GK_FAST_BUILD=1): complex64 storage only, 3x faster to compile
@@ -166,6 +186,11 @@ void stage_launch(gk_ctx *c, const GkStageArgs &A) {
     cudaEventRecord(c->ev[c->ev_used].first, c->stream);
   }
   launch_stage(c, A);
+  if (c->stage_kind == GK_KIND_POINT && A.mom) {   // this kind leaves the moment of the new state to the moment kernel
+#define GK_CALL(ST) launch_moment<ST>(c, A.out, A.mom)
+    GK_BY_STORAGE(c, GK_CALL);
+#undef GK_CALL
+  }
   if (prof) {
     cudaEventRecord(c->ev[c->ev_used].second, c->stream);
     ++c->ev_used;
@@ -174,7 +199,7 @@ void stage_launch(gk_ctx *c, const GkStageArgs &A) {
 
 int solve_phi_from_planes(gk_ctx *c, float2 *mom, float2 *phi) {
   const GkDev &P = c->P;
-  gk::gk_phi_kernel<<<(unsigned)((P.nphi + 255) / 256), 256, 0, c->stream>>>(P, mom, phi);
+  gk::gk_phi_kernel<<<(unsigned)((P.nphi + 255) / 256), 256, 0, c->stream>>>(P, mom, phi, c->d_gmax);
   ++c->launches;
   if (P.adiabatic) {
     gk::gk_zonal_kernel<<<P.nkx, 32, 0, c->stream>>>(P, phi);
@@ -243,6 +268,7 @@ int create_impl(const gk_grid *g, const gk_species *sp, const gk_salpha *geo, co
   P.ds_inv = (float)(1.0 / T.ds); P.dv_inv = (float)(1.0 / T.dv);
   P.nu_s = (float)o->disp_par; P.nu_v = (float)o->disp_vp;
   P.dkx = (float)T.dkx; P.ky0 = (float)g->ky0;
+  P.kxmax = (float)(T.K * T.dkx); P.kymax = (float)((T.nky - 1) * g->ky0);
   P.invK = T.K > 0 ? (float)(1.0 / T.K) : 0.f;
   P.invM = T.nky > 1 ? (float)(1.0 / (T.nky - 1)) : 0.f;
   P.ae = o->adiabatic_electrons ? (float)(o->ne / o->te) : 0.f;
@@ -282,6 +308,7 @@ int create_impl(const gk_grid *g, const gk_species *sp, const gk_salpha *geo, co
   const StagePick pick = gk_pick_stage(o->storage, P.mx, P.my, P.nky, P.nkx, nl);
   if (!pick.fn) return fail(c, GK_EUNSUPPORTED, "this build has no stage kernel for the requested storage");
   c->stage_fn = pick.fn;
+  c->stage_fn2 = pick.fn2;
   c->stage_threads = pick.threads;
   c->stage_kind = pick.kind;
   c->stage_cluster = pick.cluster;
@@ -312,10 +339,12 @@ int create_impl(const gk_grid *g, const gk_species *sp, const gk_salpha *geo, co
     c->stage_smem = fixed + (in_smem ? gbytes : 0) + (size_t)P.rc * P.ldy * 8;
   } else if (pick.kind == GK_KIND_GENERIC) {
     c->stage_smem = (size_t)P.slab * 8;
+  } else if (pick.kind == GK_KIND_POINT) {
+    c->stage_smem = 0;
   } else {
     c->stage_smem = pick.smem;
   }
-  {
+  if (pick.kind != GK_KIND_POINT) {
     // The attribute belongs to the kernel symbol, not to this context: the generic kernel (one symbol, plan by
     // shape) always gets the opt-in maximum so that contexts of different shapes can coexist.
     const size_t attr_smem = pick.kind == GK_KIND_GENERIC ? kSmemMax : c->stage_smem;
@@ -377,13 +406,33 @@ int create_impl(const gk_grid *g, const gk_species *sp, const gk_salpha *geo, co
     (dir ? P.twy : P.twx) = (const float2 *)p;
   }
 
+  // create-time CFL bounds and the context-owned diagnostics block
+  gkt::cfl_static(T, sp, *o, P.mask, &c->dt_lin, &c->dt_field);
+  {
+    c->part_slots = std::max(kFluxBlocks, c->stage_grid * ((c->stage_threads + 31) / 32));
+    const size_t nspec = (size_t)P.nkx + P.nky;
+    const size_t bytes = 256 + (16 + nspec + (size_t)c->part_slots * 3 * P.nsp) * sizeof(double);
+    void *p = nullptr;
+    cudaError_t e = cudaMalloc(&p, bytes);
+    if (e != cudaSuccess) return fail(c, e == cudaErrorMemoryAllocation ? GK_ENOMEM : GK_ECUDA,
+                                      std::string("cudaMalloc(diagnostics): ") + cudaGetErrorString(e));
+    c->dev_allocs.push_back(p);
+    GK_CUDA(c, cudaMemset(p, 0, bytes));
+    c->d_gmax = (unsigned int *)p;
+    c->d_flux_out = (double *)((char *)p + 256);
+    c->d_spec = c->d_flux_out + 16;
+    c->d_part = c->d_spec + nspec;
+  }
+
   // workspace layout
   size_t off = 0;
   c->off_mom = off; off += align256((size_t)P.nparts * P.nphi * 8);
   c->off_phi = off; off += align256((size_t)P.nphi * 8);
   c->off_gchi = off;
   if (nl && !P.gchi_in_smem) off += align256((size_t)c->stage_grid * P.mx * P.ldy * 8);
-  c->off_chis = off; off += align256((size_t)c->stage_grid * pick.chis_per_cta * 8);
+  c->off_chis = off;
+  off += align256(pick.kind == GK_KIND_POINT ? (size_t)P.nsp * P.nmu * P.ns * 3 * P.slab * 8
+                                              : (size_t)c->stage_grid * pick.chis_per_cta * 8);
   c->off_nl = off; off += align256((size_t)c->stage_grid * pick.nl_per_cta * 8);
   c->need_rhs = off;
   c->off_ya = off; off += align256((size_t)P.ntot * c->elem_bytes);
@@ -467,6 +516,7 @@ int gk_rhs(gk_ctx *c, const void *f, void *phi, void *rhs) {
   A.chis = (float2 *)((char *)c->ws + c->off_chis);
   A.nlbuf = (float2 *)((char *)c->ws + c->off_nl);
   A.nwork = c->stage_nwork;
+  A.gmax = c->d_gmax;
   stage_launch(c, A);
   return check_launch(c, "stage kernel");
 }
@@ -487,7 +537,9 @@ int gk_rk4_steps(gk_ctx *c, void *f, double dt, int nsteps) {
   A.chis = (float2 *)(ws + c->off_chis);
   A.nlbuf = (float2 *)(ws + c->off_nl);
   A.nwork = c->stage_nwork;
+  A.gmax = c->d_gmax;
   const float h = (float)dt;
+  const size_t part_bytes = (size_t)c->part_slots * 3 * c->P.nsp * sizeof(double);
   for (int s = 0; s < nsteps; ++s) {
     if (s == 0) {  // later steps reuse the moment planes written by the previous stage 4
 #define GK_CALL(ST) launch_moment<ST>(c, f, mom)
@@ -497,7 +549,25 @@ int gk_rk4_steps(gk_ctx *c, void *f, double dt, int nsteps) {
     // classical RK4: acc = f + dt/6 k1, then += dt/3 k2, += dt/3 k3, f = acc + dt/6 k4
     if (int r = solve_phi_from_planes(c, mom, phi)) return r;
     A.mode = 1; A.y = f; A.fn = f; A.out = ya; A.c = 0.5f * h; A.b = h / 6.f;
+    const bool fused_diag = c->diag && c->stage_kind != GK_KIND_POINT;
+    if (c->diag && !fused_diag) {   // one thread per point: no streaming role to fold the reduction into
+#define GK_CALL(ST) launch_flux<ST>(c, f, phi)
+      GK_BY_STORAGE(c, GK_CALL);
+#undef GK_CALL
+      c->flux_valid = true;
+    }
+    if (fused_diag) {   // fluxes of (f_n, phi(f_n)) from the registers of this launch's streaming role
+      GK_CUDA(c, cudaMemsetAsync(c->d_part, 0, part_bytes, c->stream));
+      A.fluxp = c->d_part;
+    }
     stage_launch(c, A);
+    if (fused_diag) {
+      A.fluxp = nullptr;
+      gk::gk_flux_sum_kernel<<<1, 32, 0, c->stream>>>(c->P, c->d_part, c->stage_grid * ((c->stage_threads + 31) / 32),
+                                                      c->d_flux_out);
+      ++c->launches;
+      c->flux_valid = true;
+    }
     if (int r = solve_phi_from_planes(c, mom, phi)) return r;
     A.mode = 2; A.y = ya; A.fn = f; A.out = yb; A.c = 0.5f * h; A.b = h / 3.f;
     stage_launch(c, A);
@@ -562,26 +632,86 @@ int gk_rk4_batch_host(gk_ctx *c, const void *const *f_in, void *const *f_out, in
   return GK_OK;
 }
 
-int gk_fluxes(gk_ctx *c, const void *f, const void *phi, double *out_host) {
-  if (int r = usable(c)) return r;
-  if (!f || !phi || !out_host) return fail(c, GK_EINVAL, "gk_fluxes: null pointer");
-  double *d = nullptr;
-  GK_CUDA(c, cudaMalloc(&d, 3 * c->P.nsp * sizeof(double)));
-  cudaMemsetAsync(d, 0, 3 * c->P.nsp * sizeof(double), c->stream);
-#define GK_CALL(ST) launch_flux<ST>(c, f, (const float2 *)phi, d)
-  GK_BY_STORAGE(c, GK_CALL);
-#undef GK_CALL
-  cudaError_t e = cudaMemcpyAsync(out_host, d, 3 * c->P.nsp * sizeof(double), cudaMemcpyDeviceToHost, c->stream);
-  if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
-  cudaFree(d);
-  if (e != cudaSuccess) return fail(c, GK_ECUDA, std::string("gk_fluxes: ") + cudaGetErrorString(e));
-  // species factors: -(1/ns) 2 pi w_v  x {1, T_a, m_a vR_a}
+namespace {
+// species factors of the flux triple: -(1/ns) 2 pi w_v  x {1, T_a, m_a vR_a}
+void flux_factors(const gk_ctx *c, double *out_host) {
   for (int a = 0; a < c->P.nsp; ++a) {
     const double base = 2.0 * gkt::kPi * c->T.wv / c->T.ns;
     out_host[3 * a + 0] *= base;
     out_host[3 * a + 1] *= base * c->species[a].temp;
     out_host[3 * a + 2] *= base * c->species[a].mass * c->T.vR[a];
   }
+}
+}  // namespace
+
+int gk_fluxes(gk_ctx *c, const void *f, const void *phi, double *out_host) {
+  if (int r = usable(c)) return r;
+  if (!f || !phi || !out_host) return fail(c, GK_EINVAL, "gk_fluxes: null pointer");
+#define GK_CALL(ST) launch_flux<ST>(c, f, (const float2 *)phi)
+  GK_BY_STORAGE(c, GK_CALL);
+#undef GK_CALL
+  c->flux_valid = false;    // the output slot now holds this call's result, not a step's
+  cudaError_t e = cudaMemcpyAsync(out_host, c->d_flux_out, 3 * c->P.nsp * sizeof(double), cudaMemcpyDeviceToHost, c->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+  if (e != cudaSuccess) return fail(c, GK_ECUDA, std::string("gk_fluxes: ") + cudaGetErrorString(e));
+  flux_factors(c, out_host);
+  return GK_OK;
+}
+
+int gk_set_diagnostics(gk_ctx *c, int on) {
+  if (int r = usable(c)) return r;
+  c->diag = on != 0;
+  if (!c->diag) c->flux_valid = false;
+  return GK_OK;
+}
+
+int gk_fluxes_last(gk_ctx *c, double *out_host) {
+  if (int r = usable(c)) return r;
+  if (!out_host) return fail(c, GK_EINVAL, "gk_fluxes_last: null pointer");
+  if (!c->flux_valid) return fail(c, GK_EINVAL, "gk_fluxes_last: no step has run with diagnostics enabled");
+  cudaError_t e = cudaMemcpyAsync(out_host, c->d_flux_out, 3 * c->P.nsp * sizeof(double), cudaMemcpyDeviceToHost, c->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+  if (e != cudaSuccess) return fail(c, GK_ECUDA, std::string("gk_fluxes_last: ") + cudaGetErrorString(e));
+  flux_factors(c, out_host);
+  return GK_OK;
+}
+
+int gk_estimate_dt(gk_ctx *c, double *out_host) {
+  if (int r = usable(c)) return r;
+  if (!out_host) return fail(c, GK_EINVAL, "gk_estimate_dt: null pointer");
+  unsigned int bits = 0;
+  cudaError_t e = cudaMemcpyAsync(&bits, c->d_gmax, sizeof(bits), cudaMemcpyDeviceToHost, c->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+  if (e != cudaSuccess) return fail(c, GK_ECUDA, std::string("gk_estimate_dt: ") + cudaGetErrorString(e));
+  float g = 0.f;
+  std::memcpy(&g, &bits, sizeof(g));
+  // R21: lambda_NL = (1/2) max(|d_y chi| kx_max + |d_x chi| ky_max); RK4 is stable on the imaginary axis to 2 sqrt 2
+  const bool nl = (c->P.mask & GK_T_III) != 0;
+  out_host[1] = (nl && g > 0.f) ? 2.0 * std::sqrt(2.0) / (0.5 * (double)g) : HUGE_VAL;
+  out_host[2] = c->dt_lin;
+  out_host[3] = c->dt_field;
+  out_host[0] = std::min(out_host[1], std::min(out_host[2], out_host[3]));
+  return GK_OK;
+}
+
+int gk_rk4_steps_cfl(gk_ctx *c, void *f, int nsteps, double safety, double dt_max, double *dt_used_host,
+                     double *t_advanced_host) {
+  if (int r = usable(c)) return r;
+  if (!f || nsteps < 0 || !(safety > 0.0)) return fail(c, GK_EINVAL, "gk_rk4_steps_cfl: bad arguments");
+  double t = 0.0;
+  for (int s = 0; s < nsteps; ++s) {
+    // one-step lag: the nonlinear bound comes from the grad(chi) of the most recent stage launch;
+    // before the first one only the linear bounds exist ("conservative linear-only estimate")
+    double est[4];
+    if (int r = gk_estimate_dt(c, est)) return r;
+    double dt = safety * est[0];
+    if (dt_max > 0.0) dt = std::min(dt, dt_max);
+    if (!(dt > 0.0) || !std::isfinite(dt)) return fail(c, GK_EINVAL, "gk_rk4_steps_cfl: no finite step (give dt_max)");
+    if (int r = gk_rk4_steps(c, f, dt, 1)) return r;
+    if (dt_used_host) dt_used_host[s] = dt;
+    t += dt;
+  }
+  if (t_advanced_host) *t_advanced_host = t;
   return GK_OK;
 }
 
@@ -589,14 +719,11 @@ int gk_spectra(gk_ctx *c, const void *phi, double *kx_spec, double *ky_spec) {
   if (int r = usable(c)) return r;
   if (!phi || !kx_spec || !ky_spec) return fail(c, GK_EINVAL, "gk_spectra: null pointer");
   const int n = c->P.nkx + c->P.nky;
-  double *d = nullptr;
-  GK_CUDA(c, cudaMalloc(&d, n * sizeof(double)));
-  gk::gk_spectra_kernel<<<n, 256, 0, c->stream>>>(c->P, (const float2 *)phi, d);
+  gk::gk_spectra_kernel<<<n, 256, 0, c->stream>>>(c->P, (const float2 *)phi, c->d_spec);
   ++c->launches;
   std::vector<double> h(n);
-  cudaError_t e = cudaMemcpyAsync(h.data(), d, n * sizeof(double), cudaMemcpyDeviceToHost, c->stream);
+  cudaError_t e = cudaMemcpyAsync(h.data(), c->d_spec, n * sizeof(double), cudaMemcpyDeviceToHost, c->stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
-  cudaFree(d);
   if (e != cudaSuccess) return fail(c, GK_ECUDA, std::string("gk_spectra: ") + cudaGetErrorString(e));
   std::memcpy(kx_spec, h.data(), c->P.nkx * sizeof(double));
   std::memcpy(ky_spec, h.data() + c->P.nkx, c->P.nky * sizeof(double));

@@ -8,7 +8,8 @@ enum {
   GK_KIND_GENERIC = 0,  // gk_stage_kernel: any shape, run-time sizes
   GK_KIND_WS2 = 2,      // gk_stage_ws2_kernel: in-place warp-specialised kernel (BASELINE grids 2-4)
   GK_KIND_LIN = 3,      // gk_stage_lin_kernel: term III off, streaming role only
-  GK_KIND_WS4 = 5       // gk_stage_ws4_kernel: 4-CTA cluster (BASELINE grid 5)
+  GK_KIND_WS4 = 5,      // gk_stage_ws4_kernel: 4-CTA cluster (BASELINE grid 5)
+  GK_KIND_POINT = 6     // gk_chis_kernel + gk_stage_point_kernel: term III off on tiny (kx,ky) planes, one thread per point
 };
 
 // smem > 0: the kernel's own fixed shared-memory plan, 0: planned by gk_create (generic kernel)
@@ -23,6 +24,7 @@ struct StagePick {
   int cluster;
   int nsh;
   size_t chis_per_cta, nl_per_cta;
+  const void *fn2 = nullptr;   // GK_KIND_POINT: gk_chis_kernel, launched before fn
 };
 
 // storage 0: complex64, 1: complex fp16, 2: complex bf16

@@ -145,7 +145,8 @@ __device__ __forceinline__ void make_epi_ptrs(const GkStageArgs &A, const SlabCt
 template <class ST, int MODE, bool INTERIOR>
 __device__ __forceinline__ float2 rhs_point(const GkDev &P, const GkStageArgs &A, const ItemCtx &I,
                                             const SlabCtx &C, const EpiPtrs<ST> &Q, int slab, int e,
-                                            int ip, int m, float pk, float fmf, float2 nlv, float scale) {
+                                            int ip, int m, float pk, float fmf, float2 nlv, float scale,
+                                            float &fsum) {
   const float2 f0 = Cv<ST>::ldg(Q.yb, e);
   float2 fs[5];
   float wsd[5];
@@ -199,6 +200,7 @@ __device__ __forceinline__ float2 rhs_point(const GkDev &P, const GkStageArgs &A
   } else if constexpr (MODE == 1) {
     Cv<ST>::stcs(Q.accb, e, gkfft::caxpy(A.b, r, f0));
     out = gkfft::caxpy(A.c, r, f0);
+    fsum = fmaf(2.f * fmf, chi0.x * f0.y - chi0.y * f0.x, fsum);   // flux diagnostics (FluxAcc)
   } else if constexpr (MODE == 2) {
     Cv<ST>::stcs(Q.accb, e, gkfft::caxpy(A.b, r, ac));
     out = gkfft::caxpy(A.c, r, fn);
@@ -333,11 +335,24 @@ gk_stage_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkStage
 
   const float scale = 0.25f * P.fftnorm;  // 1/2 (bracket) * 1/2 (two-for-one unpack) / (mx my)
 
+  // diagnostics folded into the launch (gk_common.cuh): CFL maximum of grad(chi), fluxes of the stage-1 state
+  GmaxAcc gm;
+  __shared__ double fslots[(NT / 32) * 3];
+  const bool want_flux = A.fluxp != nullptr && A.mode == 1;
+  double *fslot = fslots + (tid >> 5) * 3;
+  if ((tid & 31) == 0) fslot[0] = fslot[1] = fslot[2] = 0.0;
+  FluxAcc fx;
+  int a_prev = -1;
+
   for (int w = blockIdx.x; w < A.nwork; w += gridDim.x) {
     const int i = w % P.ns;
     const int c = (w / P.ns) % P.nchunk;
     const int al = w / (P.ns * P.nchunk);
     const int l = al % P.nmu, a = al / P.nmu;
+    if (want_flux && a != a_prev) {
+      if ((tid & 31) == 0) flux_flush(P, A.fluxp, blockIdx.x, NT / 32, tid >> 5, a_prev, fslot);
+      a_prev = a;
+    }
     ItemCtx I;
     make_item_ctx(P, a, l, i, I);
     {
@@ -348,7 +363,9 @@ gk_stage_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkStage
                 [&](int r0) {
                   for (int q = tid; q < rc * my; q += nthr) {
                     const int r = q / my, y = q - r * my;
-                    SG[(r0 + r) * ldy + y] = SW[r * ldy + y];
+                    const float2 gv = SW[r * ldy + y];
+                    SG[(r0 + r) * ldy + y] = gv;
+                    gm.add(P, gv);
                   }
                 });
       }
@@ -440,6 +457,7 @@ gk_stage_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkStage
       // are all requested before the arithmetic; the arithmetic is one packed-fp32 FMA per operand.
       EpiPtrs<ST> Q;
       make_epi_ptrs<ST>(A, C, chis, slab, Q);
+      float fsum = 0.f;
       auto point = [&](auto modec, auto intc, int e, int ip, int m, float pk, float fmf) -> float2 {
         float2 nlv = make_float2(0.f, 0.f);
         if constexpr (NL) {
@@ -447,7 +465,7 @@ gk_stage_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkStage
           nlv = SA[n * ldx + m];
         }
         return rhs_point<ST, decltype(modec)::value, decltype(intc)::value != 0>(
-            P, A, I, C, Q, slab, e, ip, m, pk, fmf, nlv, scale);
+            P, A, I, C, Q, slab, e, ip, m, pk, fmf, nlv, scale, fsum);
       };
       auto epilogue = [&](auto modec, auto intc) {
         if constexpr (ROWMAP) {
@@ -490,8 +508,10 @@ gk_stage_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkStage
         case 2: by_plane(gkfft::IC<2>{}); break;
         default: by_plane(gkfft::IC<3>{}); break;
       }
+      if (want_flux) fx.slab(P, l, i, j, fsum);
       __syncthreads();  // A / stage are rewritten by the next slab
     }
+    if (want_flux) fx.item_end(fslot);
     if (A.mom) {
       // moment plane of this item: Z n 2 pi w_v B_i w_mu J0 sum_j f   (a1 of the next stage)
       const float momw = P.sp[a].momfac * P.wmu[l] * P.B[i];
@@ -504,6 +524,8 @@ gk_stage_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkStage
       }
     }
   }
+  if constexpr (NL) gm.flush(A.gmax);
+  if (want_flux && (tid & 31) == 0) flux_flush(P, A.fluxp, blockIdx.x, NT / 32, tid >> 5, a_prev, fslot);
 }
 
 }  // namespace gk

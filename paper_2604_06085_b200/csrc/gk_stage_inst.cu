@@ -6,6 +6,7 @@
 #include "gk_epilogue.cuh"
 #include "gk_stage_ws2.cuh"
 #include "gk_stage_ws4.cuh"
+#include "gk_stage_point.cuh"
 #include "gk_pick.h"
 
 #ifndef GK_ST_ID
@@ -54,6 +55,9 @@ template <class ST> StagePick pick_stage(int mx, int my, int nky, int nkx, bool 
   GK_LIN(16, 85, 352, 1, 1);
   GK_LIN(64, 127, 512, 4, 1);
 #undef GK_LIN
+  // term III off on planes too small to occupy a CTA: one thread per grid point
+  if (!nl && slab < 256)
+    return {(const void *)gk::gk_stage_point_kernel<ST>, 256, GK_KIND_POINT, 0, 1, 1, 0, 0, (const void *)gk::gk_chis_kernel<ST>};
   if (!nl) return {(const void *)gk::gk_stage_kernel<ST, 0, 0, 0, 0, false, 512, 1>, 512, GK_KIND_GENERIC, 0, 1, 1, 3 * slab, 0};
   return {(const void *)gk::gk_stage_kernel<ST, 0, 0, 0, 0, true, 512, 1>, 512, GK_KIND_GENERIC, 0, 1, 1, 3 * slab, 0};
 }

@@ -78,7 +78,7 @@ constexpr size_t ws2_smem_bytes() {
 // in registers over the vpar march (one float2 per point of the thread).
 template <class ST, int NKY_, int NKX_, int NTF, int NTE, int NB>
 __device__ __forceinline__ void ws_epilogue_role2(const GkDev &P, const GkStageArgs &A, float2 *chis_cta,
-                                                  const float2 *nl_cta, float *eblk, int tid) {
+                                                  const float2 *nl_cta, float *eblk, double *fslots, int tid) {
   constexpr int NT = NTF + NTE;
   constexpr int nky = NKY_, nkx = NKX_;
   constexpr int K = (nkx - 1) / 2, slab = nkx * nky;
@@ -93,12 +93,21 @@ __device__ __forceinline__ void ws_epilogue_role2(const GkDev &P, const GkStageA
   const float scale = 0.25f * P.fftnorm;  // 1/2 (bracket) * 1/2 (two-for-one unpack) / (mx my)
   const long long jstride = (long long)P.nmu * P.ns * P.slab;
   const float fm2 = fmf * fmf;
-  int u = 0, it = 0;
+  // flux diagnostics of the state a stage-1 launch reads (FluxAcc, gk_common.cuh)
+  const bool want_flux = A.fluxp != nullptr && A.mode == 1;
+  double *fslot = fslots + (et >> 5) * 3;
+  if ((et & 31) == 0) fslot[0] = fslot[1] = fslot[2] = 0.0;
+  FluxAcc fx;
+  int u = 0, it = 0, a_prev = -1;
   for (int w = blockIdx.x; w < A.nwork; w += gridDim.x, ++it) {
     const int i = w % P.ns;
     const int c = (w / P.ns) % P.nchunk;
     const int al = w / (P.ns * P.nchunk);
     const int l = al % P.nmu, a = al / P.nmu;
+    if (want_flux && a != a_prev) {
+      if ((et & 31) == 0) flux_flush(P, A.fluxp, blockIdx.x, NTE / 32, et >> 5, a_prev, fslot);
+      a_prev = a;
+    }
     const long long base0 = (((long long)a * P.nv * P.nmu + l) * P.ns + i) * P.slab;
     const float2 *chip = chis_cta + (it % GK_WS_CHI_RING) * 3 * slab + et;
     // per item: kappa = -(pk ksx + m kcz), hyper-viscosity hx4 (p/K)^4 + hy4 (m/(nky-1))^4
@@ -149,6 +158,7 @@ __device__ __forceinline__ void ws_epilogue_role2(const GkDev &P, const GkStageA
       const float2 *nlr = nl_cta + (u & 1) * slab + et;
       const float2 *dsp = chip + (1 + sg) * slab;
       bar_sync_n(BAR_FULL + (u & 1), NT);   // also publishes eb to the role's other threads
+      float fsum = 0.f;
       auto sweep = [&](auto modec, auto seamc) {
         constexpr int MODE = decltype(modec)::value;
         constexpr bool SEAM = decltype(seamc)::value != 0;
@@ -221,6 +231,7 @@ __device__ __forceinline__ void ws_epilogue_role2(const GkDev &P, const GkStageA
               } else if constexpr (MODE == 1) {
                 Cv<ST>::stcs(accp, eo, gkfft::caxpy(A.b, r, f0[q]));
                 out = gkfft::caxpy(A.c, r, f0[q]);
+                fsum = fmaf(2.f * fmf, chi0[q].x * f0[q].y - chi0[q].y * f0[q].x, fsum);
               } else if constexpr (MODE == 2) {
                 Cv<ST>::stcs(accp, eo, gkfft::caxpy(A.b, r, ac[q]));
                 out = gkfft::caxpy(A.c, r, fn[q]);
@@ -244,8 +255,10 @@ __device__ __forceinline__ void ws_epilogue_role2(const GkDev &P, const GkStageA
         case 2: by_plane(gkfft::IC<2>{}); break;
         default: by_plane(gkfft::IC<3>{}); break;
       }
+      if (want_flux) fx.slab(P, l, i, j, fsum);
       bar_arrive_n(BAR_FREE + (u & 1), NT);
     }
+    if (want_flux) fx.item_end(fslot);
     if (A.mom) {
       // moment plane of this item: Z n 2 pi w_v B_i w_mu J0 sum_j f   (a1 of the next stage)
       const float momw = P.sp[a].momfac * P.wmu[l] * P.B[i];
@@ -258,6 +271,7 @@ __device__ __forceinline__ void ws_epilogue_role2(const GkDev &P, const GkStageA
       }
     }
   }
+  if (want_flux && (et & 31) == 0) flux_flush(P, A.fluxp, blockIdx.x, NTE / 32, et >> 5, a_prev, fslot);
 }
 
 // RF, RE: registers per thread of the FFT / epilogue role after setmaxnreg (0: the launch allocation is
@@ -296,6 +310,7 @@ gk_stage_ws2_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkS
   ST *stg = (ST *)sp;            // the slab being transformed, landed by the bulk copy
   uint64_t *mbar = (uint64_t *)((unsigned char *)stg + slab * sizeof(ST));
   float *eblk = (float *)(mbar + 2);  // 16-byte aligned: slab-uniform epilogue coefficients, 2 slots
+  __shared__ double fslots[(NTE / 32) * 3];
   if (tid == 0) { mbar_init(mbar, 1); mbar_init_fence(); }
   __syncthreads();
 
@@ -423,6 +438,7 @@ gk_stage_ws2_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkS
       }
     };
     // ---- Y2: inverse y pass 2, S -> dst (grad(chi) of the work item) ----
+    GmaxAcc gm;
     auto y2_to = [&](float2 *dst) {
       for (int w = tid; w < MX_ * RY2; w += NTF) {
         const int r = w % MX_, k2 = w / MX_;
@@ -433,7 +449,7 @@ gk_stage_ws2_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkS
         dft<RY1, +1>(u);
         float2 *d = dst + r * LD + k2 * RY1;
 #pragma unroll
-        for (int k1 = 0; k1 < RY1; ++k1) d[k1] = u[k1];
+        for (int k1 = 0; k1 < RY1; ++k1) { d[k1] = u[k1]; gm.add(P, u[k1]); }
       }
     };
     // ---- YF: inverse y pass 2 of rows p and p + H, bracket d_y chi d_x f - d_x chi d_y f (real space
@@ -590,9 +606,10 @@ gk_stage_ws2_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkS
     }
     // consume the epilogue's last arrivals so that no barrier is left half-way at exit
     for (int v = max(0, u - GK_WS_NL_RING); v < u; ++v) bar_sync_n(BAR_FREE + (v & 1), NT);
+    gm.flush(A.gmax);
   } else {
     if constexpr (RE > 0) asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(RE));
-    ws_epilogue_role2<ST, NKY_, NKX_, NTF, NTE, NB>(P, A, chis_cta, nl_cta, eblk, tid);
+    ws_epilogue_role2<ST, NKY_, NKX_, NTF, NTE, NB>(P, A, chis_cta, nl_cta, eblk, fslots, tid);
   }
 }
 

@@ -56,7 +56,9 @@ struct Ws4Hooks {
   uint64_t *full, *free_;  // [2] each
   float *eblk;           // [NTE/32][GK_EB_N]
   float2 *maccs;         // [EPT][NTE][PV] shared memory: moment accumulators, thread-private slots
+  double *fslots;        // [NTE/32][3]
   int et;
+  __device__ __forceinline__ double *fluxslot() const { return fslots + (et >> 5) * 3; }
   __device__ __forceinline__ float *coef(int, int t) const { return eblk + (t >> 5) * GK_EB_N; }
   __device__ __forceinline__ bool makes_coef(int t) const {
     __syncwarp();
@@ -139,6 +141,7 @@ gk_stage_ws4_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkS
   uint64_t *mbar = (uint64_t *)((unsigned char *)stg + slab * sizeof(ST));  // [0] staging, [2..3] FULL, [4..5] FREE
   uint64_t *full = mbar + 2, *free_ = mbar + 4;
   float *eblk = (float *)(mbar + 8);
+  __shared__ double fslots[(NTE / 32) * 3];
   if (tid == 0) {
     mbar_init(mbar, 1);
     mbar_init(full, CL); mbar_init(full + 1, CL);
@@ -154,6 +157,9 @@ gk_stage_ws4_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkS
     const gkfft::NamedSync<GK_WS_BAR_FFT, NTF> fsync;
     // ---- X1: folding + inverse x pass 1 of the spectral slab g (callable: slab index -> value) ----
     // h[n1] = w^{n1 q} sum_t i^{t q} (i kx -+ ky) g[n1 + MQ t]; the padding (K < n < mx - K) is never loaded
+    // The items of a warp share n1a (NC is a multiple of 32): the body is instantiated once per n1a, so that which of
+    // the CL fold terms exist, their kx and their slab rows are compile-time constants (no predicate arithmetic, no
+    // dead loads); only the rotations by the CTA rank q stay run-time (uniform).
     auto x1 = [&](auto g) {
       for (int w = tid; w < NC * RX1; w += NTF) {
         const int c = w % NC, n1a = w / NC;
@@ -163,25 +169,30 @@ gk_stage_ws4_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkS
         const int col = isp ? m : MY_ - m;
         const float kyv = isp ? -(float)m * P.ky0 : (float)m * P.ky0;
         float2 u[RX2];
-#pragma unroll
-        for (int n2 = 0; n2 < RX2; ++n2) {
-          const int n1 = n1a + RX1 * n2;
-          float2 acc = make_float2(0.f, 0.f);
-#pragma unroll
-          for (int t = 0; t < CL; ++t) {
-            const int n = n1 + MQ * t;
-            // t = 0: n < MQ <= K always retained (kx >= 0); t = CL-1: n >= mx - MQ >= mx - K always retained (kx < 0)
-            const bool pos = (t == 0) || (t < CL - 1 && n <= K);
-            const bool neg = (t == CL - 1) || (t > 0 && n >= MX_ - K);
-            if (pos || neg) {
-              const int p = pos ? n : n - MX_;
-              const float2 v = g((p + K) * NKY_ + m);
-              const float2 d = gkfft::caxpy(kyv, v, gkfft::cscale((float)p * P.dkx, make_float2(-v.y, v.x)));  // (i kx -+ ky) v
-              acc = cadd(acc, mul_ipow(d, t * q));
-            }
-          }
-          u[n2] = gkfft::cmul(acc, c_w192.w[(n1 * q) % MX_]);
-        }
+        float dkx = P.dkx;
+        int qq = q;                     // opaque copies: the products p * dkx and the twiddles w^{n1 q} are formed where
+        asm volatile("" : "+f"(dkx), "+r"(qq));   // they are used, not hoisted out of the item loop (and spilled)
+        sfor<0, RX1>([&](auto n1ac) {
+          constexpr int N1A = decltype(n1ac)::value;
+          if (n1a != N1A) return;
+          sfor<0, RX2>([&](auto n2c) {
+            constexpr int n2 = decltype(n2c)::value, n1 = N1A + RX1 * n2;
+            float2 acc = make_float2(0.f, 0.f);
+            sfor<0, CL>([&](auto tc) {
+              constexpr int t = decltype(tc)::value, n = n1 + MQ * t;
+              // t = 0: n < MQ <= K always retained (kx >= 0); t = CL-1: n >= mx - MQ >= mx - K always retained (kx < 0)
+              constexpr bool pos = (t == 0) || (t < CL - 1 && n <= K);
+              constexpr bool neg = (t == CL - 1) || (t > 0 && n >= MX_ - K);
+              if constexpr (pos || neg) {
+                constexpr int p = pos ? n : n - MX_;
+                const float2 v = g((p + K) * NKY_ + m);
+                const float2 d = gkfft::caxpy(kyv, v, gkfft::cscale((float)p * dkx, make_float2(-v.y, v.x)));  // (i kx -+ ky) v
+                acc = cadd(acc, mul_ipow(d, t * qq));
+              }
+            });
+            u[n2] = gkfft::cmul(acc, c_w192.w[(n1 * qq) % MX_]);
+          });
+        });
         dft<RX2, +1>(u);
         twiddle_row<RX2, +1>(u, tw_tab<MQ>().a + n1a * RX2);
         float2 *o = S + n1a * LD + col;
@@ -237,6 +248,7 @@ gk_stage_ws4_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkS
       }
     };
     // ---- Y2: inverse y pass 2, S -> SG (grad(chi) of the work item) ----
+    GmaxAcc gm;
     auto y2_to_sg = [&]() {
       for (int w = tid; w < MQ * RY2; w += NTF) {
         const int r = w % MQ, k2 = w / MQ;
@@ -247,7 +259,7 @@ gk_stage_ws4_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkS
         dft<RY1, +1>(u);
         float2 *d = SG + r * LD + k2 * RY1;
 #pragma unroll
-        for (int k1 = 0; k1 < RY1; ++k1) d[k1] = u[k1];
+        for (int k1 = 0; k1 < RY1; ++k1) { d[k1] = u[k1]; gm.add(P, u[k1]); }
       }
     };
     // ---- YF: inverse y pass 2 of rows p and p + H, bracket d_y chi d_x f - d_x chi d_y f (real space
@@ -338,20 +350,25 @@ gk_stage_ws4_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkS
 #pragma unroll
         for (int k2 = 0; k2 < RX2; ++k2) u[k2] = o[k2 * RX1 * LD];
         dft<RX2, -1>(u);
-#pragma unroll
-        for (int n2 = 0; n2 < RX2; ++n2) {
-          const int kap = n1 + RX1 * n2;
-#pragma unroll
-          for (int t = 0; t < CL; ++t) {
-            const int k = kap + MQ * t;
-            const bool pos = (t == 0) || (t < CL - 1 && k <= K);
-            const bool neg = (t == CL - 1) || (t > 0 && k >= MX_ - K);
-            if (pos || neg) {
-              const int p = pos ? k : k - MX_;
-              __stcg(&nlw[(p + K) * NKY_ + m], gkfft::cmulc(u[n2], c_w192.w[(k * q) % MX_]));
-            }
-          }
-        }
+        int qq = q;
+        asm volatile("" : "+r"(qq));    // see X1
+        // n1 is uniform over a warp (NKY_ is a multiple of 32): one instantiation per n1, retained kx compile-time
+        sfor<0, RX1>([&](auto n1c) {
+          constexpr int N1 = decltype(n1c)::value;
+          if (n1 != N1) return;
+          sfor<0, RX2>([&](auto n2c) {
+            constexpr int n2 = decltype(n2c)::value, kap = N1 + RX1 * n2;
+            sfor<0, CL>([&](auto tc) {
+              constexpr int t = decltype(tc)::value, k = kap + MQ * t;
+              constexpr bool pos = (t == 0) || (t < CL - 1 && k <= K);
+              constexpr bool neg = (t == CL - 1) || (t > 0 && k >= MX_ - K);
+              if constexpr (pos || neg) {
+                constexpr int p = pos ? k : k - MX_;
+                __stcg(&nlw[(p + K) * NKY_ + m], gkfft::cmulc(u[n2], c_w192.w[(k * qq) % MX_]));
+              }
+            });
+          });
+        });
       }
     };
 
@@ -411,20 +428,27 @@ gk_stage_ws4_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkS
         }
       }
     }
+    gm.flush(A.gmax);
   } else {
     // =============================== streaming role ===============================
     asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(RE));
     using HK = Ws4Hooks<ST, NKY_, NKX_, CL, NTE>;
     const int et = tid - NTF;
     HK h{A.chis + (size_t)blockIdx.x * (3 * HK::SHARE), nlring, full, free_, eblk,
-         (float2 *)(eblk + (NTE / 32) * GK_EB_N), et};
+         (float2 *)(eblk + (NTE / 32) * GK_EB_N), fslots, et};
     const int row0 = q * ROWS, nrows = min(ROWS, NKX_ - row0);
-    int u = 0;
+    const bool want_flux = A.fluxp != nullptr && A.mode == 1;
+    if ((et & 31) == 0) { double *fs = h.fluxslot(); fs[0] = fs[1] = fs[2] = 0.0; }
+    int u = 0, a_prev = -1;
     for (int w = cid; w < A.nwork; w += ncl) {
       const int i = w % P.ns;
       const int c = (w / P.ns) % P.nchunk;
       const int al = w / (P.ns * P.nchunk);
       const int l = al % P.nmu, a = al / P.nmu;
+      if (want_flux && a != a_prev) {
+        if ((et & 31) == 0) flux_flush(P, A.fluxp, blockIdx.x, NTE / 32, et >> 5, a_prev, h.fluxslot());
+        a_prev = a;
+      }
       // chi and D_s chi at the thread's own points: written and read back by the same thread (L2 scratch)
       epi_build_chis<ST, NKY_, NTE, ROWS>(P, A, a, l, i, row0, nrows, et, [&](int k, int which, const float2 (&v)[HK::M::PV]) {
         const int el = (et / HK::M::VPR + k * HK::M::RS) * NKY_ + (et % HK::M::VPR) * HK::M::PV;
@@ -434,6 +458,7 @@ gk_stage_ws4_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkS
       });
       epi_item<ST, NKY_, NKX_, NTE, ROWS, NB>(P, A, h, et, a, l, i, c, row0, nrows, u);
     }
+    if (want_flux && (et & 31) == 0) flux_flush(P, A.fluxp, blockIdx.x, NTE / 32, et >> 5, a_prev, h.fluxslot());
   }
   // no CTA leaves while its peers may still arrive at its barriers
   cluster_sync_all();

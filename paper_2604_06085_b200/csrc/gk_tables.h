@@ -2,6 +2,7 @@
 // (step a0: PAPER.md:65, 336).  Product path: its own quadrature / Bessel / geometry code,
 // nothing shared with oracle/.
 #pragma once
+#include <algorithm>
 #include <cmath>
 #include <vector>
 
@@ -179,6 +180,91 @@ inline void build_tables(const gk_grid &g, const gk_species *sp, const gk_salpha
       for (int sg = 0; sg < 2; ++sg) T.dcoef[c][sg][d] = centred ? c4[d] : up[sg][d];
       T.discoef[c][d] = centred ? d4[d] : 0.0;
     }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Create-time part of the CFL estimate (readings R22, R23 of DESIGN.md): the largest RK4-stable
+// step of (ii) the streaming and trapping stencils by a frozen-coefficient von Neumann analysis and (iii), with
+// kinetic electrons, of the electrostatic shear-Alfven (omega_H) oscillation.  No safety factor.
+// ---------------------------------------------------------------------------------------------------------------
+// |R(z)|^2 of classical RK4, R(z) = 1 + z + z^2/2 + z^3/6 + z^4/24
+inline double rk4_gain2(double zr, double zi) {
+  // Horner in complex arithmetic written out
+  double ar = 1.0 / 24.0, ai = 0.0;
+  const double c[4] = {1.0 / 6.0, 0.5, 1.0, 1.0};
+  for (int k = 0; k < 4; ++k) {
+    const double tr = ar * zr - ai * zi + c[k], ti = ar * zi + ai * zr;
+    ar = tr; ai = ti;
+  }
+  return ar * ar + ai * ai;
+}
+// first tau > 0 at which the ray {tau z} leaves the stability region |R| <= 1
+inline double rk4_first_exit(double zr, double zi) {
+  const double az = std::hypot(zr, zi);
+  if (az == 0.0) return HUGE_VAL;
+  const double tmax = 4.0 / az;
+  const int n = 4096;
+  double lo = 0.0, hi = -1.0;
+  for (int k = 1; k <= n; ++k) {
+    const double t = tmax * k / n;
+    if (rk4_gain2(t * zr, t * zi) > 1.0 + 1e-13) { hi = t; break; }
+    lo = t;
+  }
+  if (hi < 0.0) return tmax;
+  for (int it = 0; it < 100; ++it) {
+    const double mid = 0.5 * (lo + hi);
+    (rk4_gain2(mid * zr, mid * zi) > 1.0 + 1e-13 ? hi : lo) = mid;
+  }
+  return lo;
+}
+inline void cfl_static(const Tables &T, const gk_species *sp, const gk_opts &o, int mask, double *dt_lin,
+                       double *dt_field) {
+  // (ii) z(t, t') = c_s [-i sigma(t) - nu_s d(t)] + c_v [+i sigma(t') - nu_v d(t')], 64 x 64 angles
+  double cs = 0.0, cv = 0.0;
+  for (int a = 0; a < T.nsp; ++a)
+    for (int i = 0; i < T.ns; ++i) {
+      cs = std::max(cs, std::fabs(T.vR[a] * T.F[i]) * std::max(std::fabs(T.v.front()), std::fabs(T.v.back())) / T.ds);
+      cv = std::max(cv, std::fabs(T.vR[a] * T.BG[i]) * T.mu.back() / T.dv);
+    }
+  for (int l = 0; l < T.nmu; ++l)   // the mu grid is increasing for both grid types; keep the scan honest anyway
+    for (int a = 0; a < T.nsp; ++a)
+      for (int i = 0; i < T.ns; ++i) cv = std::max(cv, std::fabs(T.vR[a] * T.mu[l] * T.BG[i]) / T.dv);
+  if (!(mask & GK_T_I)) cs = 0.0;
+  if (!(mask & GK_T_IV)) cv = 0.0;
+  const double nus = (mask & GK_T_DISS_S) ? o.disp_par : 0.0, nuv = (mask & GK_T_DISS_V) ? o.disp_vp : 0.0;
+  double best = HUGE_VAL;
+  const int NA = 64;
+  double sg[NA], d4[NA];
+  for (int k = 0; k < NA; ++k) {
+    const double t = 2.0 * kPi * k / NA;
+    sg[k] = (8.0 * std::sin(t) - std::sin(2.0 * t)) / 6.0;
+    d4[k] = (2.0 - 2.0 * std::cos(t)) * (2.0 - 2.0 * std::cos(t)) / 12.0;
+  }
+  for (int k1 = 0; k1 < NA; ++k1)
+    for (int k2 = 0; k2 < NA; ++k2)
+      best = std::min(best, rk4_first_exit(-cs * nus * d4[k1] - cv * nuv * d4[k2], -cs * sg[k1] + cv * sg[k2]));
+  *dt_lin = best;
+  // (iii) omega_H^2 = sum_a (v_R F k_s)^2 Z^2 n <v_par^2> / (T A), <v_par^2> = 1/2, k_s = max sigma / ds;
+  // max sigma in closed form: cos t = 1 - sqrt(6)/2
+  *dt_field = HUGE_VAL;
+  if (!o.adiabatic_electrons && (mask & GK_T_I) && (mask & GK_T_VII)) {
+    const double ct = 1.0 - std::sqrt(6.0) / 2.0, st = std::sqrt(1.0 - ct * ct);
+    const double ks = (8.0 * st - 2.0 * st * ct) / 6.0 / T.ds;
+    double om2 = 0.0;
+    for (int i = 0; i < T.ns; ++i) {
+      double num = 0.0;
+      for (int a = 0; a < T.nsp; ++a) {
+        const double c = T.vR[a] * T.F[i] * ks;
+        num += c * c * sp[a].Z * sp[a].Z * sp[a].dens * 0.5 / sp[a].temp;
+      }
+      for (int ip = 0; ip < T.nkx; ++ip)
+        for (int m = 0; m < T.nky; ++m) {
+          if (ip == T.K && m == 0) continue;
+          om2 = std::max(om2, num / T.den[((size_t)i * T.nkx + ip) * T.nky + m]);
+        }
+    }
+    if (om2 > 0.0) *dt_field = 2.0 * std::sqrt(2.0) / std::sqrt(om2);
+  }
 }
 
 }  // namespace gkt

@@ -1,5 +1,5 @@
 """CPU-side checks of the boundary: the C-ABI library builds/loads, exports every symbol that
-include/gk.h declares, and refuses to work without a CUDA device (no CPU fallback)."""
+include/*.h declare, and refuses to work without a CUDA device (no CPU fallback)."""
 import ctypes as C
 import os
 import subprocess
@@ -15,7 +15,8 @@ def test_library_loads_and_exports_every_declared_symbol():
     names = binding.exported_symbols()
     assert {"gk_create", "gk_destroy", "gk_field_solve", "gk_rhs", "gk_rk4_step", "gk_rk4_steps",
             "gk_fluxes", "gk_workspace_bytes", "gk_set_workspace", "gk_export_table",
-            "gk_last_error"} <= set(names)
+            "gk_last_error", "gk_estimate_dt", "gk_rk4_steps_cfl", "gk_set_diagnostics", "gk_fluxes_last",
+            "gk_spectra", "gk_launch_count", "gk_stage_kernel_time"} <= set(names)
     for n in names:
         assert hasattr(lib, n), n
     assert b"sm_100a" in lib.gk_version()
