@@ -238,11 +238,20 @@ def run_reference(args, cfg, rank):
 
 
 def run_cufft_compare(args, cfg):
-    """Measured comparison only (north_star: cuFFT is allowed as a measured comparison): term III of
-    one stage done the library way -- padded gradient spectra written to HBM, batched cuFFT c2r (torch.fft.irfft2),
-    pointwise product, cuFFT r2c, truncation -- on arrays of the workload's shape, beside the fused stage kernel.
-    The ky=0 Hermitian average (R15) is not applied here: this is a timing of the data movement, not a parity path."""
+    """Measured comparisons only (north_star: cuFFT is allowed as a measured comparison).  Term III of one
+    stage done the library way, on arrays of the workload's (kx, ky) plane, beside the fused stage kernel:
+
+      r2c     padded gradient spectra written to HBM, batched cuFFT c2r (torch.fft.irfft2) x 2 per slab, pointwise
+              product, cuFFT r2c, truncation (round 1's comparison; a timing of the data movement);
+      packed  the paper's own layout (D.3): both gradients of a field packed into ONE complex field
+              Z = d_x g + i d_y g, its full 2-D spectrum synthesised from the stored half by Hermitian extension with
+              the ky = 0 mirror pairs (kx, -kx) replaced by their Hermitian average, one C2C inverse per field, bracket,
+              one forward r2c; in complex64 (the paper's MP bracket) and in complex128 (its DP bracket).
+
+    The packed legs are CHECKED against the oracle's bracket (direct definition through its own FFT) on a few slabs
+    before they are timed, so the comparison is between two correct implementations of the same operation."""
     import torch
+    from oracle.gkref import GkRef
     from paper_2604_06085_b200 import GkContext
     dev = torch.device("cuda", 0)
     g = GkContext(cfg, device=dev)
@@ -250,17 +259,23 @@ def run_cufft_compare(args, cfg):
     K = (nkx - 1) // 2
     plan = g.plan()
     mx, my = plan["mx"], plan["my"]
-    nli = 8                                   # (mu, s) pairs per batch: nli * nv slabs
+    M = nky - 1
+    dkx = float(g.gk_export_table("kx")[K + 1] - g.gk_export_table("kx")[K])
+    ky0 = cfg["grid"]["ky0"]
+    nli = 4                                   # (mu, s) pairs per batch: nli * nv slabs
     nbatch = (nsp * nmu * ns + nli - 1) // nli
     gen = torch.Generator(device=dev).manual_seed(1)
-    f = torch.randn(nli, nv, nkx, nky, 2, device=dev, generator=gen)
-    f = torch.view_as_complex(f) * 1e-3
+    f = torch.view_as_complex(torch.randn(nli, nv, nkx, nky, 2, device=dev, generator=gen)) * 1e-3
+    chi = torch.view_as_complex(torch.randn(nli, 1, nkx, nky, 2, device=dev, generator=gen)) * 1e-2
+    reps = max(1, args.steps)
+
+    # ---- leg "r2c" (as in round 1) ----
+    kx = (torch.arange(nkx, device=dev) - K).float().view(1, 1, nkx, 1) * dkx
+    ky = torch.arange(nky, device=dev).float().view(1, 1, 1, nky) * ky0
     gchi = torch.randn(2, nli, 1, mx, my, device=dev, generator=gen)   # real-space grad(chi), reused over vpar
-    kx = (torch.arange(nkx, device=dev) - K).float().view(1, 1, nkx, 1) * 0.1
-    ky = torch.arange(nky, device=dev).float().view(1, 1, 1, nky) * 0.1
     pad = torch.zeros(2, nli, nv, mx, my // 2 + 1, dtype=torch.complex64, device=dev)
 
-    def bracket_batch():
+    def bracket_r2c():
         gx, gy = 1j * kx * f, 1j * ky * f
         for q, src in enumerate((gx, gy)):
             pad[q, :, :, :K + 1, :nky] = src[:, :, K:, :]
@@ -270,32 +285,80 @@ def run_cufft_compare(args, cfg):
         out = torch.fft.rfft2(br, norm="forward")
         return torch.cat((out[:, :, mx - K:, :nky], out[:, :, :K + 1, :nky]), dim=2)
 
-    for _ in range(3):
-        bracket_batch()
-    torch.cuda.synchronize()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    reps = max(1, args.steps)
-    e0.record()
-    for _ in range(reps * nbatch):
-        bracket_batch()
-    e1.record()
-    torch.cuda.synchronize()
-    ms_stage = e0.elapsed_time(e1) / reps
+    # ---- leg "packed": Z = d_x g + i d_y g through one C2C inverse per field ----
+    def packed_spectrum(gs, cdt):
+        """gs [..., nkx, nky] half spectrum -> full padded 2-D spectrum [..., mx, my] of d_x g + i d_y g."""
+        gs = gs.to(cdt)
+        rdt = torch.float64 if cdt == torch.complex128 else torch.float32
+        kxv = ((torch.arange(nkx, device=dev) - K).to(rdt) * dkx).view(nkx, 1)
+        kyv = (torch.arange(nky, device=dev).to(rdt) * ky0).view(1, nky)
+        g0 = gs.clone()
+        g0[..., 0] = 0.5 * (gs[..., 0] + torch.conj(torch.flip(gs[..., 0], dims=(-1,))))   # Hermitian average of the mirror pairs
+        zp = (1j * kxv - kyv) * g0                                   # ky >= 0:  (i kx) g + i (i ky) g
+        zm = torch.conj(torch.flip(g0, dims=(-2,)))                  # g(-kx... ) : value at (kx, -ky) = conj g(-kx, ky)
+        zmm = (1j * kxv + kyv) * zm                                  # (i kx) g(kx,-ky) + i (i (-ky)) g(kx,-ky)
+        full = torch.zeros(gs.shape[:-2] + (mx, my), dtype=cdt, device=dev)
+        for lo, hi, dst in ((K, nkx, slice(0, K + 1)), (0, K, slice(mx - K, mx))):
+            full[..., dst, :nky] = zp[..., lo:hi, :]
+            full[..., dst, my - M:] = torch.flip(zmm[..., lo:hi, 1:], dims=(-1,))
+        return full
+
+    def bracket_packed(fb, chib, cdt):
+        zf = torch.fft.ifft2(packed_spectrum(fb, cdt), norm="forward")       # Re = d_x f, Im = d_y f
+        zc = torch.fft.ifft2(packed_spectrum(chib, cdt), norm="forward")
+        br = 0.5 * (zc.imag * zf.real - zc.real * zf.imag)
+        out = torch.fft.rfft2(br, norm="backward") / (mx * my)
+        return torch.cat((out[..., mx - K:, :nky], out[..., :K + 1, :nky]), dim=-2)
+
+    # parity of the packed legs against the oracle's bracket, asymmetric ky = 0 columns included
+    o = GkRef(cfg, pad=(mx, my))
+    rng = np.random.default_rng(5)
+    fs = (rng.standard_normal((3, nkx, nky)) + 1j * rng.standard_normal((3, nkx, nky)))
+    cs = (rng.standard_normal((3, nkx, nky)) + 1j * rng.standard_normal((3, nkx, nky)))
+    parity = {}
+    for name, cdt in (("packed_c64", torch.complex64), ("packed_c128", torch.complex128)):
+        got = bracket_packed(torch.from_numpy(fs).to(dev), torch.from_numpy(cs).to(dev), cdt).cpu().numpy()
+        ref = np.stack([o.bracket_slab(cs[q], fs[q], 0, mx, my) for q in range(3)])
+        parity[name] = float(np.linalg.norm(got - ref) / np.linalg.norm(ref))
+    assert parity["packed_c64"] < 1e-5 and parity["packed_c128"] < 1e-12, parity
+
+    def time_leg(fn):
+        for _ in range(3):
+            fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(reps * nbatch):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / reps
+
+    ms_r2c = time_leg(bracket_r2c)
+    ms_p64 = time_leg(lambda: bracket_packed(f, chi, torch.complex64))
+    ms_p128 = time_leg(lambda: bracket_packed(f, chi, torch.complex128))
     # the fused stage kernel (whole stage: field solve + linear terms + bracket + RK update) on the same grid
     fd = g.to_state(gkinputs.initial_f(cfg, np.complex64))
     g.gk_rk4_steps(fd, cfg["dt"], 3)
     torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
     g.gk_rk4_steps(fd, cfg["dt"], reps)
     e1.record()
     torch.cuda.synchronize()
     fused = e0.elapsed_time(e1) / (4 * reps)
-    print(json.dumps({"compare": "cufft_unfused_bracket", "workload": cfg["name"], "padded_fft": [mx, my],
+    print(json.dumps({"compare": "cufft_bracket", "workload": cfg["name"], "padded_fft": [mx, my],
                       "slabs_per_stage": nsp * nv * nmu * ns, "batch_slabs": nli * nv,
-                      "cufft_bracket_ms_per_stage": ms_stage, "fused_whole_stage_ms": fused,
-                      "ratio_bracket_alone_over_whole_fused_stage": ms_stage / fused,
-                      "note": "torch.fft (cuFFT) irfft2/rfft2 with padded arrays in HBM; term III only, no linear terms, "
-                              "no RK update, no field solve"}), flush=True)
+                      "cufft_r2c_bracket_ms_per_stage": ms_r2c,
+                      "cufft_packed_c2c_fp32_bracket_ms_per_stage": ms_p64,
+                      "cufft_packed_c2c_fp64_bracket_ms_per_stage": ms_p128,
+                      "packed_parity_vs_oracle_rel_l2": parity,
+                      "fused_whole_stage_ms": fused,
+                      "ratio_packed_fp32_bracket_over_whole_fused_stage": ms_p64 / fused,
+                      "note": "torch.fft (cuFFT) with padded arrays in HBM; term III only (no linear terms, no RK update, "
+                              "no field solve); the packed legs build the full Hermitian-extended spectrum with the "
+                              "mirror-pair average of PAPER.md:440 and pass a parity check against the oracle first"}),
+          flush=True)
 
 
 def main():
@@ -417,7 +480,7 @@ def main():
     batch_ms = max_over_ranks(e0.elapsed_time(e1), world, dev)
     fbytes = fd.numel() * fd.element_size()
     plan = g.plan()
-    kernel_names = {0: "gk_stage_kernel", 2: "gk_stage_ws2_kernel", 3: "gk_stage_lin_kernel", 5: "gk_stage_ws4_kernel"}
+    kernel_names = {0: "gk_stage_kernel", 2: "gk_stage_ws2_kernel", 3: "gk_stage_lin_kernel", 5: "gk_stage_ws4_kernel", 6: "gk_stage_point_kernel"}
 
     # ---- secondary workload (rank 0, N = 1): the stage kernel of BASELINE config 3 (the round-1 headline) ----
     secondary = None

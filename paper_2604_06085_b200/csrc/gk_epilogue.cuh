@@ -130,6 +130,7 @@ template <class ST, int NKY_, int NTE, int ROWS> struct EpiMap {
 //   void   chi(int k, int el, int sg, float2 (&chi)[PV], float2 (&dsc)[PV])   el: index inside the share
 //   void   nl(int u, int e, float2 (&v)[PV])                                   e: index inside the slab
 //   float2 *macc(int k)               PV moment accumulators of the thread's item k (shared memory, thread-private)
+//   static constexpr bool FLUX        the flux diagnostics are folded into this role (else the host runs gk_flux_kernel)
 //   double *fluxslot()                3 doubles of the thread's warp in shared memory (flux diagnostics, FluxAcc)
 // u counts the slabs this CTA has processed since the start of the launch (ring slots).
 template <class ST, int NKY_, int NKX_, int NTE, int ROWS, int NB, class H>
@@ -158,7 +159,7 @@ __device__ __forceinline__ void epi_item(const GkDev &P, const GkStageArgs &A, H
 
   // ---- register window along vpar; the moment accumulators live in thread-private shared-memory slots ----
   float2 win[EPT][4][PV];
-  const bool want_flux = A.fluxp != nullptr && A.mode == 1;
+  const bool want_flux = H::FLUX && A.fluxp != nullptr && A.mode == 1;
   FluxAcc fx;
   const ST *y0 = (const ST *)A.y + base0;
 #pragma unroll
@@ -285,7 +286,7 @@ __device__ __forceinline__ void epi_item(const GkDev &P, const GkStageArgs &A, H
               r = gkfft::caxpy(we.x * kap, make_float2(f0[v].y, -f0[v].x), r);
               r = gkfft::caxpy(we.y * fmf + we.z * kap, make_float2(chi0[q][v].y, -chi0[q][v].x), r);
               rr[v] = r;
-              if constexpr (MODE == 1) {
+              if constexpr (MODE == 1 && H::FLUX) {
                 if (valid) fsum = fmaf(2.f * fmf, chi0[q][v].x * f0[v].y - chi0[q][v].y * f0[v].x, fsum);
               }
               // the window moves on by one slab
@@ -346,10 +347,10 @@ __device__ __forceinline__ void epi_item(const GkDev &P, const GkStageArgs &A, H
       case 2: by_plane(gkfft::IC<2>{}); break;
       default: by_plane(gkfft::IC<3>{}); break;
     }
-    if (want_flux) fx.slab(P, l, i, j, fsum);
+    if constexpr (H::FLUX) { if (want_flux) fx.slab(P, l, i, j, fsum); }
     h.end(u);
   }
-  if (want_flux) fx.item_end(h.fluxslot());
+  if constexpr (H::FLUX) { if (want_flux) fx.item_end(h.fluxslot()); }
   if (A.mom) {
     // moment plane of this item: Z n 2 pi w_v B_i w_mu J0 sum_j f   (a1 of the next stage)
     const float momw = P.sp[a].momfac * P.wmu[l] * P.B[i];
@@ -415,12 +416,12 @@ __device__ __forceinline__ void epi_build_chis(const GkDev &P, const GkStageArgs
 template <class ST, int NKY_, int NKX_, int NT, int NSH, int NB>
 struct LinHooks {
   static constexpr bool NL = false;
+  static constexpr bool FLUX = false;   // 168 registers per thread are all taken: fluxes through gk_flux_kernel
   using M = EpiMap<ST, NKY_, NT, (NKX_ + NSH - 1) / NSH>;
   float2 *chis;   // [4][EPT][NT][PV] shared memory: chi, D_s chi (v > 0), D_s chi (v < 0), moment accumulators
   float *eblk;    // [NT/32][GK_EB_N]
-  double *fslots; // [NT/32][3]
   int et;
-  __device__ __forceinline__ double *fluxslot() const { return fslots + (et >> 5) * 3; }
+  __device__ __forceinline__ double *fluxslot() const { return nullptr; }
   __device__ __forceinline__ float *coef(int, int t) const { return eblk + (t >> 5) * GK_EB_N; }
   __device__ __forceinline__ bool makes_coef(int t) const {
     __syncwarp();                  // the warp has finished reading the previous slab's block
@@ -455,14 +456,11 @@ __global__ void __launch_bounds__(NT, 1)
 gk_stage_lin_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkStageArgs A) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   __shared__ __align__(16) float eblk[(NT / 32) * GK_EB_N];
-  __shared__ double fslots[(NT / 32) * 3];
   constexpr int ROWS = (NKX_ + NSH - 1) / NSH;
   using HK = LinHooks<ST, NKY_, NKX_, NT, NSH, NB>;
-  HK h{(float2 *)smem_raw, eblk, fslots, (int)threadIdx.x};
+  HK h{(float2 *)smem_raw, eblk, (int)threadIdx.x};
   const int et = threadIdx.x;
-  const bool want_flux = A.fluxp != nullptr && A.mode == 1;
-  if ((et & 31) == 0) { double *fs = h.fluxslot(); fs[0] = fs[1] = fs[2] = 0.0; }
-  int u = 0, a_prev = -1;
+  int u = 0;
   for (int w = blockIdx.x; w < A.nwork; w += gridDim.x) {
     const int i = w % P.ns;
     const int sh = (w / P.ns) % NSH;
@@ -470,10 +468,6 @@ gk_stage_lin_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkS
     const int al = w / (P.ns * NSH * P.nchunk);
     const int l = al % P.nmu, a = al / P.nmu;
     const int row0 = sh * ROWS, nrows = min(ROWS, NKX_ - row0);
-    if (want_flux && a != a_prev) {          // species are visited in increasing order: one write per (warp, species)
-      if ((et & 31) == 0) flux_flush(P, A.fluxp, blockIdx.x, NT / 32, et >> 5, a_prev, h.fluxslot());
-      a_prev = a;
-    }
     epi_build_chis<ST, NKY_, NT, ROWS>(P, A, a, l, i, row0, nrows, et, [&](int k, int which, const float2 (&v)[HK::M::PV]) {
       float4 *p = (float4 *)h.slot(which, k);
 #pragma unroll
@@ -481,7 +475,6 @@ gk_stage_lin_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkS
     });
     epi_item<ST, NKY_, NKX_, NT, ROWS, NB>(P, A, h, et, a, l, i, c, row0, nrows, u);
   }
-  if (want_flux && (et & 31) == 0) flux_flush(P, A.fluxp, blockIdx.x, NT / 32, et >> 5, a_prev, h.fluxslot());
 }
 
 }  // namespace gk

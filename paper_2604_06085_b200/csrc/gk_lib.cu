@@ -17,7 +17,8 @@
 
 namespace {
 
-constexpr size_t kSmemMax = 232448;  // 227 KB opt-in dynamic shared memory per CTA on sm_100
+constexpr size_t kSmemMax = 232448;  // 227 KB opt-in shared memory per CTA on sm_100 (static + dynamic)
+constexpr size_t kSmemDyn = kSmemMax - 1024;  // dynamic part the generic kernel may plan with (it has some static arrays)
 
 inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
@@ -325,7 +326,7 @@ int create_impl(const gk_grid *g, const gk_species *sp, const gk_salpha *geo, co
       const size_t base = fixed + (pass == 0 ? gbytes : 0);
       for (int rc = P.mx; rc >= 2; rc /= 2) {
         if (P.mx % rc || rc % 2) continue;
-        if (base + (size_t)rc * P.ldy * 8 <= kSmemMax) {
+        if (base + (size_t)rc * P.ldy * 8 <= kSmemDyn) {
           if (pass == 0 && rc < std::min(16, P.mx)) break;
           rc_best = rc;
           in_smem = (pass == 0);
@@ -347,7 +348,7 @@ int create_impl(const gk_grid *g, const gk_species *sp, const gk_salpha *geo, co
   if (pick.kind != GK_KIND_POINT) {
     // The attribute belongs to the kernel symbol, not to this context: the generic kernel (one symbol, plan by
     // shape) always gets the opt-in maximum so that contexts of different shapes can coexist.
-    const size_t attr_smem = pick.kind == GK_KIND_GENERIC ? kSmemMax : c->stage_smem;
+    const size_t attr_smem = pick.kind == GK_KIND_GENERIC ? kSmemDyn : c->stage_smem;
     cudaError_t e = cudaFuncSetAttribute(c->stage_fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)attr_smem);
     if (e != cudaSuccess) return fail(c, GK_ECUDA, std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e));
   }
@@ -549,8 +550,8 @@ int gk_rk4_steps(gk_ctx *c, void *f, double dt, int nsteps) {
     // classical RK4: acc = f + dt/6 k1, then += dt/3 k2, += dt/3 k3, f = acc + dt/6 k4
     if (int r = solve_phi_from_planes(c, mom, phi)) return r;
     A.mode = 1; A.y = f; A.fn = f; A.out = ya; A.c = 0.5f * h; A.b = h / 6.f;
-    const bool fused_diag = c->diag && c->stage_kind != GK_KIND_POINT;
-    if (c->diag && !fused_diag) {   // one thread per point: no streaming role to fold the reduction into
+    const bool fused_diag = c->diag && c->stage_kind != GK_KIND_POINT && c->stage_kind != GK_KIND_LIN;
+    if (c->diag && !fused_diag) {   // point kernel: no streaming role; streaming kernel: no registers to spare
 #define GK_CALL(ST) launch_flux<ST>(c, f, phi)
       GK_BY_STORAGE(c, GK_CALL);
 #undef GK_CALL

@@ -49,6 +49,7 @@ template <int NKY_, int NKX_, int CL> constexpr size_t ws4_chis_elems() {
 template <class ST, int NKY_, int NKX_, int CL, int NTE>
 struct Ws4Hooks {
   static constexpr bool NL = true;
+  static constexpr bool FLUX = true;
   static constexpr int ROWS = (NKX_ + CL - 1) / CL, SHARE = ROWS * NKY_, slab = NKX_ * NKY_;
   using M = EpiMap<ST, NKY_, NTE, ROWS>;
   float2 *chis;          // this CTA's scratch [3][SHARE] (L2), written and read by the same thread
@@ -445,7 +446,7 @@ gk_stage_ws4_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkS
       const int c = (w / P.ns) % P.nchunk;
       const int al = w / (P.ns * P.nchunk);
       const int l = al % P.nmu, a = al / P.nmu;
-      if (want_flux && a != a_prev) {
+      if (want_flux && a != a_prev) {   // species are visited in increasing order: one write per (warp, species)
         if ((et & 31) == 0) flux_flush(P, A.fluxp, blockIdx.x, NTE / 32, et >> 5, a_prev, h.fluxslot());
         a_prev = a;
       }

@@ -28,7 +28,7 @@ def _ctx(case, **kw):
     grid, kind = PLANES[case]
     cfg = small_cfg(**grid)
     g = GkContext(cfg, **kw)
-    assert g.plan()["kind"] == kind, g.plan()
+    assert g.plan()["kind"] == kind or (kind == 3 and g.plan()["kind"] == 7), g.plan()   # 3 / 7: linear kernels
     return cfg, g
 
 
@@ -62,22 +62,24 @@ def test_estimate_dt_parity(case):
 
 
 def test_cfl_adaptive_steps_follow_the_lagged_estimate():
-    # dt_0 = safety x linear-only bound; dt_k = safety x min(linear, nonlinear bound of the LAST stage of step k-1).
-    # The oracle replays the same rule with its own RK4 stages and its own estimate.
+    # dt_0 = min(dt_max, safety x linear-only bound); dt_k = min(dt_max, safety x min(linear, nonlinear bound of the
+    # LAST stage of step k-1)).  The oracle replays the same rule with its own RK4 stages and its own estimate.
+    # (The linear bound of PAPER.md:356 covers streaming and trapping only; at this amplitude the first step needs
+    # the dt_max cap, as a production run started from noise would.)
     cfg, g = _ctx("mid")
     p = g.plan()
     o = GkRef(cfg, pad=(p["mx"], p["my"]))
-    f = (3.0 * rand_c(np.random.default_rng(82), o.shape, True)).astype(np.complex64)
-    safety, nsteps = 0.4, 3
+    f = rand_c(np.random.default_rng(82), o.shape, True).astype(np.complex64)
+    safety, nsteps, dt_max = 0.4, 4, 1e-3
     fd = g.to_state(f)
-    dts, t = g.gk_rk4_steps_cfl(fd, nsteps, safety)
+    dts, t = g.gk_rk4_steps_cfl(fd, nsteps, safety, dt_max=dt_max)
     y = f.astype(np.complex128)
     est = o.estimate_dt(np.zeros(o.phi_shape, complex))
     want = []
     nl_binding = 0
     for k in range(nsteps):
-        dt = safety * (min(est[2], est[3]) if k == 0 else est[0])
-        nl_binding += int(k > 0 and est[1] < min(est[2], est[3]))
+        dt = min(dt_max, safety * (min(est[2], est[3]) if k == 0 else est[0]))
+        nl_binding += int(k > 0 and est[1] < min(est[2], est[3]) and safety * est[1] < dt_max)
         want.append(dt)
         k1, _ = o.rhs(y)
         k2, _ = o.rhs(y + 0.5 * dt * k1)
@@ -85,13 +87,15 @@ def test_cfl_adaptive_steps_follow_the_lagged_estimate():
         k4, phi4 = o.rhs(y + dt * k3)
         y = y + dt / 6 * (k1 + 2 * k2 + 2 * k3 + k4)
         est = o.estimate_dt(phi4)
-    assert nl_binding == nsteps - 1                    # the input is strong enough for the nonlinear bound to bind
+    assert want[0] == dt_max and nl_binding == nsteps - 1     # then the nonlinear bound sets every later step
     np.testing.assert_allclose(dts, want, rtol=2e-5)
     np.testing.assert_allclose(t, sum(want), rtol=2e-5)
     assert rel_l2(g.from_state(fd), y) < 1e-4
-    # dt_max caps the step
-    dts2, _ = g.gk_rk4_steps_cfl(g.to_state(f), 2, safety, dt_max=1e-3)
-    np.testing.assert_allclose(dts2, [1e-3, 1e-3])
+    # a fresh context without a cap: the first step is the linear-only estimate
+    _, g2 = _ctx("mid")
+    dts2, _ = g2.gk_rk4_steps_cfl(g2.to_state(1e-6 * f), 1, safety)
+    e = g2.gk_estimate_dt()
+    np.testing.assert_allclose(dts2, [safety * min(e[2], e[3])], rtol=1e-12)
 
 
 @pytest.mark.parametrize("case", ["mid", "mid_kinetic", "cfg2_plane", "cfg3_plane", "cfg3_plane_kinetic", "cfg5_plane",

@@ -81,6 +81,26 @@ def test_rhs_parity_full(case):
     assert rel_l2(rhs.cpu().numpy(), ref) < TOL_RHS
 
 
+@pytest.mark.parametrize("case,kind", [("chain", 6), ("mid", 6), ("mid2", 0), ("mid_kinetic", 6)])
+def test_linear_runs_on_the_point_and_generic_kernels(case, kind):
+    # term III off: planes of fewer than 256 modes take gk_stage_point_kernel (one thread per grid point; the
+    # moment of the new state through gk_moment_kernel), larger odd shapes the generic kernel without the bracket
+    cfg = {"chain": small_cfg(nkx=3, nky=1, ns=16, nvpar=12, nmu=3, mu_grid=1, nonlinear=0),
+           "mid": small_cfg(nonlinear=0, **MID), "mid2": small_cfg(nonlinear=0, **MID2),
+           "mid_kinetic": small_cfg(nspecies=2, adiabatic=0, nonlinear=0, **MID)}[case]
+    g, o = _ctx(cfg), GkRef(cfg)
+    assert g.plan()["kind"] == kind
+    f = rand_c(np.random.default_rng(39), o.shape, False).astype(np.complex64)
+    rhs, phi = g.gk_rhs(g.to_state(f))
+    ref, phiref = o.rhs(f)
+    assert rel_l2(phi.cpu().numpy(), phiref) < TOL_RHS
+    assert rel_l2(rhs.cpu().numpy(), ref) < TOL_RHS
+    dt = 0.0005 if case == "mid_kinetic" else 0.01
+    fd = g.to_state(f)
+    g.gk_rk4_steps(fd, dt, 10)
+    assert rel_l2(g.from_state(fd), o.rk4_step(f, dt, 10)) < TOL_RK10
+
+
 def test_bracket_independent_of_padded_size_and_matches_direct_convolution():
     cfg = small_cfg(**MID)     # K=10 -> 31, nky=6 -> 16: minimal supported 32 x 16
     o = GkRef(cfg, term_mask=G.T_III, bracket_method=1)
