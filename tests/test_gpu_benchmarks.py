@@ -72,3 +72,101 @@ def test_rosenbluth_hinton_epsilon_scan(eps):
     theory = rh_theory(q, eps)
     print(f"RH eps={eps}: residual {res:.5f} (fit constant {const:.5f}) theory {theory:.5f} ratio {res / theory:.4f}")
     assert abs(res / theory - 1) < 0.06, (res, theory)
+
+
+# ---- Cyclone base case, linear ITG: q = 1.4, shat = 0.78, eps = 0.19, R/LT = 6.9, R/Ln = 2.2,
+# adiabatic electrons, s-alpha; nperiod = 5 (the ky > 0 chain spans 2 nperiod - 1 = 9 poloidal turns = 9 connected kx),
+# Nv = 64, Nmu = 16, 160 points along the extended field line (here 18 per turn x 9), nu_par = 1.0, dt = 0.003,
+# growth rate averaged over windows of naverage = 100 steps.  The paper's reference values are GKW's and are not
+# printed, so the GPU path is compared with (a) the eigenvalues of the oracle's operator on a reduced grid and
+# (b) the qualitative content of Figure 5 at the paper's resolution (values recorded in DESIGN.md).
+def cbc_cfg(ky, rlt=6.9, ns=18, nv=64, nmu=16, nkx=9):
+    cfg = small_cfg(nkx=nkx, nky=2, ns=ns, nvpar=nv, nmu=nmu, mu_grid=1, ky0=ky, ikxspace=1, nonlinear=0,
+                    disp_par=1.0, disp_vp=0.0, disp_x=0.0, disp_y=0.0)
+    cfg["geom"].update(q=1.4, shat=0.78, eps=0.19)
+    cfg["species"][0].update(rlt=rlt, rln=2.2)
+    return cfg
+
+
+def cbc_run(cfg, dt, nwin, naverage=100, seed=5):
+    """ln sqrt(sum |phi(ky)|^2) at the end of every window of `naverage` steps, and the complex phi at the midplane."""
+    from paper_2604_06085_b200 import GkContext
+    g = GkContext(cfg)
+    assert g.plan()["kind"] == 6
+    rng = np.random.default_rng(seed)
+    f = np.zeros(g.shape, np.complex64)
+    f[..., 1] = 1e-6 * (rng.standard_normal(g.shape[:-1]) + 1j * rng.standard_normal(g.shape[:-1]))
+    fd = g.to_state(f)
+    amp, mid = [], []
+    K, ns = (g.shape[4] - 1) // 2, g.shape[3]
+    for _ in range(nwin):
+        g.gk_rk4_steps(fd, dt, naverage)
+        phi = g.gk_field_solve(fd)[:, :, 1]
+        amp.append(0.5 * float(torch_log_sum(phi)))
+        mid.append(complex(phi[ns // 2, K].item()))
+        if amp[-1] > 40:                               # renormalise before fp32 overflows
+            fd *= float(np.exp(-amp[-1]))
+            amp_shift = amp[-1]
+            amp = [a - amp_shift for a in amp]
+            mid = [m * np.exp(-amp_shift) for m in mid]
+    return np.array(amp), np.array(mid), g
+
+
+def torch_log_sum(phi):
+    import torch
+    return torch.log((phi.real.double() ** 2 + phi.imag.double() ** 2).sum())
+
+
+def growth_and_frequency(amp, mid, dt_win):
+    """gamma from a straight-line fit of the log amplitude over the second half of the run; omega from the phase
+    advance of phi at the outboard midplane per window."""
+    n = len(amp)
+    t = np.arange(n) * dt_win
+    h = slice(n // 2, n)
+    gamma = np.polyfit(t[h], amp[h], 1)[0]
+    dphase = np.angle(mid[1:] / mid[:-1])
+    omega = -np.median(dphase[n // 2:]) / dt_win        # phi ~ exp(-i omega t)
+    return gamma, omega
+
+
+def test_cbc_growth_rate_equals_the_operators_eigenvalue():
+    from oracle.gkref import GkRef
+    from tests.test_oracle_physics import _operator_matrix
+    cfg = cbc_cfg(0.4, ns=8, nv=12, nmu=3, nkx=5)
+    o = GkRef(cfg)
+    sel = np.zeros(o.shape, bool)
+    sel[..., 1] = True
+    lam = np.linalg.eigvals(_operator_matrix(o, sel))
+    dt, nav = 0.01, 50
+    z = lam * dt
+    Rz = 1 + z + z ** 2 / 2 + z ** 3 / 6 + z ** 4 / 24
+    k = np.argmax(abs(Rz))
+    assert lam[k].real > 0.02                                     # CBC at k_theta rho = 0.4 is ITG unstable
+    amp, mid, _ = cbc_run(cfg, dt, 80, naverage=nav)
+    gamma, omega = growth_and_frequency(amp, mid, dt * nav)
+    # per-step amplification of RK4 on the operator's most amplified eigenvalue, and its phase
+    np.testing.assert_allclose(gamma, np.log(abs(Rz[k])) / dt, rtol=2e-3)
+    np.testing.assert_allclose(omega, -np.angle(Rz[k]) / dt, rtol=5e-3)
+
+
+def test_cyclone_base_case_scans_at_the_papers_resolution():
+    dt, nwin, nav = 0.003, 120, 100                               # t = 36 (the paper runs 300 windows)
+    kys = [0.1, 0.2, 0.3, 0.4, 0.5, 0.6, 0.7, 0.8]
+    gam = {}
+    for ky in kys:
+        amp, mid, _ = cbc_run(cbc_cfg(ky), dt, nwin, nav)
+        gam[ky] = growth_and_frequency(amp, mid, dt * nav)
+    print("CBC R/LT=6.9: " + ", ".join(f"ky={k}: gamma={g:.4f} omega={w:.4f}" for k, (g, w) in gam.items()))
+    g = np.array([gam[k][0] for k in kys])
+    kmax = kys[int(np.argmax(g))]
+    assert 0.3 <= kmax <= 0.6 and g.max() > 0.1                   # Figure 5a: the ITG spectrum peaks near 0.4-0.5
+    assert all(gam[k][0] > 0 for k in (0.2, 0.3, 0.4, 0.5, 0.6))
+    assert all(gam[k][1] < 0 for k in (0.3, 0.4, 0.5)) or all(gam[k][1] > 0 for k in (0.3, 0.4, 0.5))   # one drift direction
+    rlts = [6.9, 8.28, 10.35, 12.44, 15.18]
+    gr = []
+    for rlt in rlts:
+        amp, mid, _ = cbc_run(cbc_cfg(0.5, rlt=rlt), dt, nwin, nav)
+        gr.append(growth_and_frequency(amp, mid, dt * nav)[0])
+    print("CBC ky=0.5: " + ", ".join(f"R/LT={r}: gamma={g:.4f}" for r, g in zip(rlts, gr)))
+    assert all(b > a for a, b in zip(gr, gr[1:]))                 # Figure 5b: gamma rises with the drive
+    np.testing.assert_allclose(gr[0], gam[0.5][0], rtol=1e-3)     # same case, same answer
