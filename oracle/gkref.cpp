@@ -132,6 +132,11 @@ struct gkref {
   double wv;
   // s-alpha geometry (R2): B, F=ffun, BG = B*gfun, sin(theta), cz = cos+shat*theta*sin, R
   std::vector<double> B, F, BG, sth, cz, R;
+  // metric of k_perp^2 = kx^2 + 2 kx ky gpz + ky^2 gzz (g_psipsi = 1 in both models; ky in k_theta rho units, i.e.
+  // g_psizeta / kthnorm and g_zetazeta / kthnorm^2) and the ExB factor ef = 2 E^{psi zeta} / kthnorm
+  // (1 in s-alpha: the factor 1/2 of terms III and V, R2)
+  std::vector<double> gpz, gzz, ef;
+  double kthnorm;
   // species tables
   std::vector<double> vR;                 // sqrt(T/m)
   std::vector<double> J0;                 // [a][l][i][p][m] (R4)
@@ -151,9 +156,8 @@ struct gkref {
   size_t jidx(int a, int l, int i, int ip, int m) const {
     return ((((size_t)a * nmu + l) * ns + i) * nkx + ip) * nky + m;
   }
-  double kperp2(int i, int ip, int m) const {  // eq. 2 with the s-alpha metric (R2)
-    double kxl = kx[ip] + geo.shat * theta[i] * ky[m];
-    return kxl * kxl + ky[m] * ky[m];
+  double kperp2(int i, int ip, int m) const {  // eq. 2 (s-alpha metric: R2)
+    return kx[ip] * kx[ip] + 2.0 * kx[ip] * ky[m] * gpz[i] + ky[m] * ky[m] * gzz[i];
   }
   double kappa(int i, int ip, int m) const {  // kx D^psi + k_zeta D^zeta (R2)
     return -(kx[ip] * sth[i] + ky[m] * cz[i]);
@@ -231,25 +235,81 @@ void gkref::build() {
       wmu[l] = vp * dvp;
     }
   }
-  dkx = 2.0 * PI * geo.shat * g.ky0 / g.ikxspace;
+  // --- geometry ---
+  B.resize(ns); F.resize(ns); BG.resize(ns); sth.resize(ns); cz.resize(ns); R.resize(ns);
+  gpz.resize(ns); gzz.resize(ns); ef.resize(ns);
+  double kxshift = 2.0 * PI * geo.shat;  // kx gained per poloidal turn, per unit ky
+  if (o.geometry == 0) {
+    // s-alpha (R2)
+    kthnorm = geo.q / (2.0 * PI * geo.eps);
+    for (int i = 0; i < ns; ++i) {
+      double th = theta[i];
+      R[i] = 1.0 + geo.eps * std::cos(th);
+      B[i] = 1.0 / R[i];
+      F[i] = 1.0 / (2.0 * PI * geo.q);                    // ffun  (eps->0 form)
+      // gfun = F * d_s B / B;  d_s B = 2 pi eps sin(th) B^2  =>  B*gfun:
+      BG[i] = (geo.eps / geo.q) * std::sin(th) * B[i] * B[i];
+      sth[i] = std::sin(th);
+      cz[i] = std::cos(th) + geo.shat * th * std::sin(th);
+      gpz[i] = geo.shat * th;
+      gzz[i] = 1.0 + geo.shat * geo.shat * th * th;
+      ef[i] = 1.0;
+    }
+  } else {
+    // Circular concentric (Lapillonne) model, reading R24.  Coordinates (R0 = 1): R = 1 + eps cos th,
+    // Z = eps sin th, psi = eps, s = (th + eps sin th)/2pi, zeta = -phi/2pi + (q/pi) A,
+    // A = atan[ sqrt((1-eps)/(1+eps)) tan(th/2) ] (the "branch-tracked arctan"), q' = shat q/eps.
+    // Closed forms of the partial derivatives; gradients: |grad eps| = 1, grad th = e_th/eps, grad phi = e_phi/R.
+    const double q = geo.q, eps = geo.eps, sq = std::sqrt(1.0 - eps * eps), dq = geo.shat * q / eps;
+    auto point = [&](double th, double *out) {
+      const double c = std::cos(th), sn = std::sin(th), Rr = 1.0 + eps * c;
+      // B = delta / (1 + eps cos th), delta^2 = 1 + eps^2/(q^2 (1 - eps^2))                         (eq. 1)
+      const double w = q * q * (1.0 - eps * eps), dw = 2.0 * q * dq * (1.0 - eps * eps) - 2.0 * eps * q * q;
+      const double del = std::sqrt(1.0 + eps * eps / w);
+      const double ddel = (2.0 * eps * w - eps * eps * dw) / (w * w) / (2.0 * del);
+      const double Bv = del / Rr, B_th = del * eps * sn / (Rr * Rr), B_eps = ddel / Rr - del * c / (Rr * Rr);
+      const double B_s = 2.0 * PI / Rr * B_th, B_psi = B_eps - sn / Rr * B_th;                    // eq. 3
+      const double A = std::atan(std::sqrt((1.0 - eps) / (1.0 + eps)) * std::tan(0.5 * th));
+      const double z_th = (q / PI) * sq / (2.0 * Rr);
+      const double z_eps = (dq / PI) * A - (q / PI) * sn / (2.0 * sq * Rr);
+      const double g_pz = z_eps, g_zz = 1.0 / (4.0 * PI * PI * Rr * Rr) + z_eps * z_eps + z_th * z_th / (eps * eps);
+      const double g_ps = sn / (2.0 * PI), g_zs = z_eps * sn / (2.0 * PI) + z_th * Rr / (2.0 * PI * eps * eps);
+      // E tensor: antisymmetric cofactors of the first two metric rows x pi dpf/dpsi / B^2
+      const double pref = PI * (eps / (q * sq)) / (Bv * Bv);
+      const double Epz = pref * (g_zz - g_pz * g_pz), Eps = pref * (g_zs - g_ps * g_pz), Ezs = pref * (g_pz * g_zs - g_ps * g_zz);
+      out[0] = Bv; out[1] = B_s; out[2] = g_pz; out[3] = g_zz;
+      out[4] = -2.0 * Eps * B_s / Bv;                                   // D^psi                   (eq. 4)
+      out[5] = -2.0 * (-Epz * B_psi + Ezs * B_s) / Bv;                  // D^zeta
+      out[6] = Epz; out[7] = Rr; out[8] = 1.0 / del;                    // bt_frac
+    };
+    double p0[9];
+    point(0.0, p0);
+    kthnorm = std::sqrt(p0[3]);
+    kxshift = dq / kthnorm;   // g_psizeta grows by q' per turn (A -> A + pi): the chain is continuous with this shift
+    for (int i = 0; i < ns; ++i) {
+      // invert th + eps sin th = 2 pi s (Newton)
+      double th = 2.0 * PI * s[i];
+      for (int it = 0; it < 50; ++it) th -= (th + eps * std::sin(th) - 2.0 * PI * s[i]) / (1.0 + eps * std::cos(th));
+      theta[i] = th;
+      double pt[9];
+      point(th, pt);
+      B[i] = pt[0];
+      F[i] = 1.0 / (2.0 * PI * q * sq) / pt[0];                         // ffun = b_ups / B
+      BG[i] = F[i] * pt[1];                                             // B gfun = F d_s B
+      gpz[i] = pt[2] / kthnorm;
+      gzz[i] = pt[3] / (kthnorm * kthnorm);
+      sth[i] = -pt[4];                                                  // kappa = kx D^psi + k_zeta D^zeta, k_zeta = ky/kthnorm
+      cz[i] = -pt[5] / kthnorm;
+      ef[i] = 2.0 * pt[6] / kthnorm;                                    // E^{psi zeta} k_zeta = ef ky / 2
+      R[i] = pt[7] * pt[8];                                             // R B_t/B of the momentum flux (R18)
+    }
+  }
+  dkx = kxshift * g.ky0 / g.ikxspace;
   kx.resize(nkx); ky.resize(nky);
   for (int ip = 0; ip < nkx; ++ip) kx[ip] = (ip - K) * dkx;
   for (int m = 0; m < nky; ++m) ky[m] = m * g.ky0;
   kxmax = K * dkx;
   kymax = (nky - 1) * g.ky0;
-
-  // --- s-alpha geometry (R2) ---
-  B.resize(ns); F.resize(ns); BG.resize(ns); sth.resize(ns); cz.resize(ns); R.resize(ns);
-  for (int i = 0; i < ns; ++i) {
-    double th = theta[i];
-    R[i] = 1.0 + geo.eps * std::cos(th);
-    B[i] = 1.0 / R[i];
-    F[i] = 1.0 / (2.0 * PI * geo.q);                    // ffun  (eps->0 form)
-    // gfun = F * d_s B / B;  d_s B = 2 pi eps sin(th) B^2  =>  B*gfun:
-    BG[i] = (geo.eps / geo.q) * std::sin(th) * B[i] * B[i];
-    sth[i] = std::sin(th);
-    cz[i] = std::cos(th) + geo.shat * th * std::sin(th);
-  }
 
   // --- species tables ---
   vR.resize(nsp);
@@ -398,7 +458,7 @@ cplx gkref::linear_point(const cplx *f, const cplx *phi, int a, int j, int l, in
 
   if (on(GKREF_T_II)) r += -I1 * (S.temp / S.Z) * ED * kap * f0;        // II  -i k.v_D f
   if (on(GKREF_T_V))                                                    // V   -v_E . grad F_M
-    r += -I1 * (0.5 * ky[m]) * chi0 * fm * (S.rln + (E - 1.5) * S.rlt);
+    r += -I1 * (0.5 * ef[i] * ky[m]) * chi0 * fm * (S.rln + (E - 1.5) * S.rlt);   // E^{psi zeta} k_zeta = ef ky/2
   if (on(GKREF_T_VIII)) r += -I1 * ED * kap * chi0 * fm;                // VIII
   if (on(GKREF_T_HYP)) {                                                // hyper-viscosity (R9)
     double hx = (kxmax > 0) ? std::pow(kx[ip] / kxmax, 4) : 0.0;
@@ -495,7 +555,7 @@ void gkref::rhs_slab(const cplx *f, const cplx *phi, int a, int j, int l, int i,
     for (int ip = 0; ip < nkx; ++ip)
       for (int m = 0; m < nky; ++m) chi[(size_t)ip * nky + m] = J0[jidx(a, l, i, ip, m)] * phi[pidx(i, ip, m)];
     bracket(chi.data(), &f[fidx(a, j, l, i, 0, 0)], o.bracket_method, o.pad_mx, o.pad_my, nl.data());
-    for (size_t n = 0; n < nslab(); ++n) out[n] += nl[n];
+    for (size_t n = 0; n < nslab(); ++n) out[n] += ef[i] * nl[n];   // the bracket carries the same ExB factor
   }
 }
 
@@ -581,7 +641,7 @@ void gkref_fluxes(const gkref *h, const double *f_in, const double *phi_in, doub
               cplx chi = h->J0[h->jidx(a, l, i, ip, m)] * phi[h->pidx(i, ip, m)];
               double im = std::imag(std::conj(chi) * f[h->fidx(a, j, l, i, ip, m)]);
               double P = (m == 0) ? 1.0 : 2.0;
-              double w = -(1.0 / h->ns) * P * 0.5 * h->ky[m] * 2.0 * PI * h->B[i] * h->wv * h->wmu[l] * im;
+              double w = -(1.0 / h->ns) * P * 0.5 * h->ef[i] * h->ky[m] * 2.0 * PI * h->B[i] * h->wv * h->wmu[l] * im;
               double E = h->v[j] * h->v[j] + 2.0 * h->mu[l] * h->B[i];
               acc[0] += w;
               acc[1] += w * E * h->sp[a].temp;
@@ -705,7 +765,7 @@ void gkref_estimate_dt(const gkref *h, const double *phi_in, double *out) {
           fft2d(gx, mx, my, +1);
           fft2d(gy, mx, my, +1);
           for (size_t n = 0; n < gx.size(); ++n) {
-            double lam = 0.5 * (std::fabs(gy[n].real()) * h->kxmax + std::fabs(gx[n].real()) * h->kymax);
+            double lam = 0.5 * h->ef[i] * (std::fabs(gy[n].real()) * h->kxmax + std::fabs(gx[n].real()) * h->kymax);
             lamnl = std::max(lamnl, lam);
           }
         }
@@ -782,6 +842,13 @@ size_t gkref_table(const gkref *h, const char *which, double *out) {
   else if (w == "Gamma0") src = &h->G0;
   else if (w == "FM") src = &h->FM;
   else if (w == "Apol") src = &h->Apol;
+  else if (w == "ef") src = &h->ef;
+  else if (w == "gpz") src = &h->gpz;
+  else if (w == "gzz") src = &h->gzz;
+  else if (w == "sth") src = &h->sth;
+  else if (w == "cz") src = &h->cz;
+  else if (w == "kthnorm") { tmp = {h->kthnorm}; src = &tmp; }
+  else if (w == "dkx") { tmp = {h->dkx}; src = &tmp; }
   else if (w == "wv") { tmp = {h->wv}; src = &tmp; }
   else if (w == "kperp2" || w == "kappa" || w == "sclass") {
     tmp.resize(h->nphi());

@@ -36,7 +36,7 @@ typedef struct {
 } gkref_grid;
 
 typedef struct { double Z, mass, temp, dens, rlt, rln; } gkref_species;
-typedef struct { double q, shat, eps; } gkref_geom; /* s-alpha (reading R2) */
+typedef struct { double q, shat, eps; } gkref_geom; /* equilibrium scalars of both geometry models */
 
 /* term_mask bits (test hook, "switch terms on one at a time") */
 enum {
@@ -55,6 +55,7 @@ typedef struct {
   int term_mask;           /* <=0: all terms                                             */
   int bracket_method;      /* 0 = padded FFT (own FFT), 1 = direct O(N^2) convolution    */
   int pad_mx, pad_my;      /* 0 = smallest 7-smooth size >= the 3/2-rule minimum (R14)   */
+  int geometry;            /* 0 s-alpha (R2), 1 circular (eq. 1-4; R24) */
 } gkref_opts;
 
 gkref *gkref_create(const gkref_grid *, const gkref_species *, const gkref_geom *,

@@ -50,7 +50,7 @@ class _Opts(C.Structure):
                 ("ne", C.c_double), ("nonlinear", C.c_int), ("disp_par", C.c_double),
                 ("disp_vp", C.c_double), ("disp_x", C.c_double), ("disp_y", C.c_double),
                 ("s_closure", C.c_int), ("term_mask", C.c_int), ("bracket_method", C.c_int),
-                ("pad_mx", C.c_int), ("pad_my", C.c_int)]
+                ("pad_mx", C.c_int), ("pad_my", C.c_int), ("geometry", C.c_int)]
 
 
 _lib = None
@@ -106,7 +106,7 @@ class GkRef:
         geo = _Geom(cfg["geom"]["q"], cfg["geom"]["shat"], cfg["geom"]["eps"])
         opts = _Opts(self.nsp, o["adiabatic_electrons"], o["te"], o["ne"], o["nonlinear"],
                      o["disp_par"], o["disp_vp"], o["disp_x"], o["disp_y"], o["s_closure"],
-                     term_mask, bracket_method, pad[0], pad[1])
+                     term_mask, bracket_method, pad[0], pad[1], int(o.get("geometry", 0)))
         self._h = lib.gkref_create(C.byref(grid), sp, C.byref(geo), C.byref(opts))
         if not self._h:
             raise ValueError("gkref_create rejected the configuration")
@@ -188,4 +188,5 @@ class GkRef:
                   "FM": (g["nvpar"], g["nmu"], g["ns"]),
                   "Apol": self.phi_shape, "kperp2": self.phi_shape, "kappa": self.phi_shape,
                   "sclass": self.phi_shape, "dcoef": (5, 2, 5)}
+        # further names: "ef" (ExB factor relative to ky/2), "gpz", "gzz" (normalised metric), "kthnorm", "dkx"
         return out.reshape(shapes.get(which, (n,)))
