@@ -44,7 +44,8 @@ typedef struct {
  * to the reference species) and the gradient drives R/L_T, R/L_n. */
 typedef struct { double Z, mass, temp, dens, rlt, rln; } gk_species;
 
-/* s-alpha geometry (formulas: reading R2). */
+/* Equilibrium scalars of the geometry model chosen by gk_opts.geometry: s-alpha (formulas:
+ * reading R2) or circular (R24). */
 typedef struct { double q, shat, eps; } gk_salpha;
 
 /* term_mask bits: debugging/test hook that switches individual terms of the RHS. */
@@ -65,6 +66,8 @@ typedef struct {
   int term_mask;           /* <= 0: all terms                                                     */
   int pad_mx, pad_my;      /* padded real-space grid of the bracket; 0 = automatic (R14).  Must be
                               >= 3K+1 / 3(nky-1)+1 and of the form 2^a * 3^b, b <= 1, <= 256      */
+  int geometry;            /* 0: s-alpha (R2); 1: circular concentric (Lapillonne) model from (q, shat, eps),
+                              PAPER.md:286-310 eq. 1-4 (R24)                                        */
 } gk_opts;
 
 /* Builds all create-time tables (grids, weights, geometry, F_M, J0, Gamma0, Poisson denominators,
@@ -158,7 +161,8 @@ int gk_rk4_steps_cfl(gk_ctx *ctx, void *f_dev, int nsteps, double safety, double
 int gk_spectra(gk_ctx *ctx, const void *phi_dev, double *kx_spec_host, double *ky_spec_host);
 
 /* Test hook: copies a create-time table to host memory as doubles.  `which` is one of
- * "vpar","mu","wmu","kx","ky","B","F","BG","J0","Gamma0","FM","den","zonal","pad".  Returns the
+ * "vpar","mu","wmu","kx","ky","B","F","BG","J0","Gamma0","FM","den","zonal","pad","ef","gpz","gzz","sth","cz","R",
+ * "kthnorm","dkx".  Returns the
  * number of doubles (also when host_out is NULL), 0 for an unknown name. */
 size_t gk_export_table(const gk_ctx *ctx, const char *which, double *host_out, size_t max_doubles);
 

@@ -42,7 +42,7 @@ class _Opts(C.Structure):
                 ("ne", C.c_double), ("nonlinear", C.c_int), ("disp_par", C.c_double),
                 ("disp_vp", C.c_double), ("disp_x", C.c_double), ("disp_y", C.c_double),
                 ("s_closure", C.c_int), ("storage", C.c_int), ("term_mask", C.c_int),
-                ("pad_mx", C.c_int), ("pad_my", C.c_int)]
+                ("pad_mx", C.c_int), ("pad_my", C.c_int), ("geometry", C.c_int)]
 
 
 def lib_path() -> str:
@@ -135,7 +135,7 @@ class GkContext:
         geo = _Salpha(cfg["geom"]["q"], cfg["geom"]["shat"], cfg["geom"]["eps"])
         opts = _Opts(self.nsp, o["adiabatic_electrons"], o["te"], o["ne"], o["nonlinear"],
                      o["disp_par"], o["disp_vp"], o["disp_x"], o["disp_y"], o["s_closure"],
-                     self.storage, term_mask, pad[0], pad[1])
+                     self.storage, term_mask, pad[0], pad[1], int(o.get("geometry", 0)))
         self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
         h = C.c_void_p()
         rc = self.lib.gk_create(C.byref(grid), sp, C.byref(geo), C.byref(opts),

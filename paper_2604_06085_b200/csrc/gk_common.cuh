@@ -64,7 +64,8 @@ template <> __device__ __forceinline__ float2 as_stored<__nv_bfloat162>(float2 v
 // |d_y chi| kx_max + |d_x chi| ky_max it has seen; one atomicMax per warp at the end of its role.
 struct GmaxAcc {
   float v = 0.f;
-  __device__ __forceinline__ void add(const GkDev &P, float2 g) { v = fmaxf(v, fabsf(g.y) * P.kxmax + fabsf(g.x) * P.kymax); }
+  // ef: ExB factor of the plane the gradient belongs to
+  __device__ __forceinline__ void add(const GkDev &P, float2 g, float ef) { v = fmaxf(v, ef * (fabsf(g.y) * P.kxmax + fabsf(g.x) * P.kymax)); }
   // all 32 lanes of the warp call
   __device__ __forceinline__ void flush(unsigned int *dst) const {
     if (!dst) return;
@@ -82,7 +83,7 @@ struct FluxAcc {
   // psum = sum over the thread's points of 2 m Im[conj(chi) f]
   __device__ __forceinline__ void slab(const GkDev &P, int l, int i, int j, float psum) {
     const float vj = P.v[j], Bi = P.B[i];
-    const float t = -0.5f * P.ky0 * Bi * P.wmu[l] * psum;
+    const float t = -0.5f * P.ef[i] * P.ky0 * Bi * P.wmu[l] * psum;
     s0 += t;
     s1 = fmaf(t, vj * vj + 2.f * P.mu[l] * Bi, s1);
     s2 = fmaf(t, vj * P.Rmaj[i], s2);

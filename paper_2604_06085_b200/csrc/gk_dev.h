@@ -40,7 +40,8 @@ struct GkDev {
   const float *v, *fmv;             // [nv]  vpar_j, pi^-3/2 exp(-v^2)
   const float *mu, *wmu;            // [nmu]
   const float *fmm;                 // [nmu][ns] exp(-2 mu B)
-  const float *B, *F, *BG, *sth, *cz, *Rmaj;  // [ns]
+  const float *B, *F, *BG, *sth, *cz, *Rmaj;  // [ns]  (sth, cz: kappa = -(kx sth + ky cz); Rmaj: R B_t/B)
+  const float *ef;                  // [ns] ExB factor of terms III, V and of the fluxes relative to ky/2 (1 in s-alpha)
   const float *kx, *ky;             // [nkx], [nky]
   const float *hypx, *hypy;         // nu_x (kx/kxmax)^4, nu_y (ky/kymax)^4
   const float *J0;                  // [nsp][nmu][ns][nkx][nky]

@@ -105,7 +105,7 @@ __device__ __forceinline__ void epi_coefficients(const GkDev &P, int a, int l, i
   eb[GK_EB_WVC] = cDv * 0.5f;
   eb[GK_EB_C7] = (mask & GK_T_VII) ? -Sp.ZoverT * cpar * fm * P.ds_inv : 0.f;
   eb[GK_EB_A2] = (mask & GK_T_II) ? Sp.ToverZ * ED : 0.f;
-  eb[GK_EB_A5] = (mask & GK_T_V) ? 0.5f * fm * (Sp.rln + (E - 1.5f) * Sp.rlt) * P.ky0 : 0.f;
+  eb[GK_EB_A5] = (mask & GK_T_V) ? 0.5f * P.ef[i] * fm * (Sp.rln + (E - 1.5f) * Sp.rlt) * P.ky0 : 0.f;
   eb[GK_EB_A8] = (mask & GK_T_VIII) ? ED * fm : 0.f;
 }
 
@@ -145,7 +145,7 @@ __device__ __forceinline__ void epi_item(const GkDev &P, const GkStageArgs &A, H
   const int el0 = r0 * nky + m0;              // index of item 0 inside the share
   const int e0 = row0 * nky + el0;            // ... inside the slab
   const int ip0 = row0 + r0;                  // kx row of item 0
-  const float scale = 0.25f * P.fftnorm;      // 1/2 (bracket) * 1/2 (two-for-one unpack) / (mx my)
+  const float scale = 0.25f * P.ef[i] * P.fftnorm;      // ef/2 (bracket) * 1/2 (two-for-one unpack) / (mx my)
   const long long jstride = (long long)P.nmu * P.ns * P.slab;
   const int js = (int)jstride;
   const long long base0 = (((long long)a * P.nv * P.nmu + l) * P.ns + i) * P.slab + e0;

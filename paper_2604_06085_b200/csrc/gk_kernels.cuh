@@ -101,7 +101,7 @@ __global__ void __launch_bounds__(256) gk_flux_kernel(const __grid_constant__ Gk
     const float2 ph = phi[(long long)i * P.slab + e];
     const float im = j0 * (ph.x * fv.y - ph.y * fv.x);  // Im[conj(chi) f]
     const float pw = (m == 0) ? 1.f : 2.f;
-    const float wgt = -pw * 0.5f * P.ky[m] * P.B[i] * P.wmu[l] * im;
+    const float wgt = -pw * 0.5f * P.ef[i] * P.ky[m] * P.B[i] * P.wmu[l] * im;
     const float vj = P.v[j];
     const float E = vj * vj + 2.f * P.mu[l] * P.B[i];
     acc[0] += wgt;

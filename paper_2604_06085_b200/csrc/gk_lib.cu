@@ -233,7 +233,8 @@ int create_impl(const gk_grid *g, const gk_species *sp, const gk_salpha *geo, co
   *out = nullptr;
   if (g->nkx < 1 || g->nkx % 2 == 0 || g->ns < 4 || g->nvpar < 4 || g->nky < 1 || g->nmu < 1 ||
       g->ikxspace < 1 || o->nspecies < 1 || o->nspecies > GK_MAX_SPECIES || o->storage < 0 ||
-      o->storage > 2 || !(g->vpar_max > 0) || (g->mu_grid != 0 && g->mu_grid != 1))
+      o->storage > 2 || !(g->vpar_max > 0) || (g->mu_grid != 0 && g->mu_grid != 1) ||
+      (o->geometry != 0 && o->geometry != 1) || !(geo->eps > 0) || !(geo->eps < 1) || !(geo->q > 0))
     return GK_EINVAL;
   for (int a = 0; a < o->nspecies; ++a)
     if (sp[a].Z == 0 || !(sp[a].mass > 0) || !(sp[a].temp > 0)) return GK_EINVAL;
@@ -391,7 +392,7 @@ int create_impl(const gk_grid *g, const gk_species *sp, const gk_salpha *geo, co
 #define UP(T_, field, vec) if ((rcode = upload<T_>(c, vec, &P.field)) != GK_OK) return rcode
   UP(float, v, T.v); UP(float, fmv, T.fmv); UP(float, mu, T.mu); UP(float, wmu, T.wmu);
   UP(float, fmm, T.fmm); UP(float, B, T.B); UP(float, F, T.F); UP(float, BG, T.BG);
-  UP(float, sth, T.sth); UP(float, cz, T.cz); UP(float, Rmaj, T.Rmaj); UP(float, kx, T.kx);
+  UP(float, sth, T.sth); UP(float, cz, T.cz); UP(float, Rmaj, T.Rmaj); UP(float, ef, T.ef); UP(float, kx, T.kx);
   UP(float, ky, T.ky); UP(float, hypx, T.hypx); UP(float, hypy, T.hypy); UP(float, J0, T.J0);
   UP(float, dinv, T.dinv); UP(float, zinv, T.zinv);
 #undef UP
@@ -740,6 +741,9 @@ size_t gk_export_table(const gk_ctx *c, const char *which, double *out, size_t m
   if (w == "vpar") src = &T.v; else if (w == "mu") src = &T.mu; else if (w == "wmu") src = &T.wmu;
   else if (w == "kx") src = &T.kx; else if (w == "ky") src = &T.ky; else if (w == "B") src = &T.B;
   else if (w == "F") src = &T.F; else if (w == "BG") src = &T.BG; else if (w == "J0") src = &T.J0;
+  else if (w == "ef") src = &T.ef; else if (w == "gpz") src = &T.gpz; else if (w == "gzz") src = &T.gzz;
+  else if (w == "sth") src = &T.sth; else if (w == "cz") src = &T.cz; else if (w == "R") src = &T.Rmaj;
+  else if (w == "kthnorm") { tmp = {T.kthnorm}; src = &tmp; } else if (w == "dkx") { tmp = {T.dkx}; src = &tmp; }
   else if (w == "Gamma0") src = &T.G0; else if (w == "den") src = &T.den; else if (w == "zonal") src = &T.zinv;
   else if (w == "FM") {
     tmp.resize((size_t)T.nv * T.nmu * T.ns);

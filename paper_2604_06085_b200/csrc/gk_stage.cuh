@@ -78,7 +78,7 @@ __device__ __forceinline__ void make_slab_ctx(const GkDev &P, const ItemCtx &I, 
   const float c4 = (mask & GK_T_IV) ? I.cmir * P.dv_inv : 0.f;
   const float cDv = (mask & GK_T_DISS_V) ? -P.nu_v * fabsf(I.cmir) * P.dv_inv : 0.f;
   C.a2 = (mask & GK_T_II) ? I.ToverZ * ED : 0.f;
-  C.a5 = (mask & GK_T_V) ? 0.5f * fm * (I.rln + (E - 1.5f) * I.rlt) : 0.f;
+  C.a5 = (mask & GK_T_V) ? 0.5f * P.ef[I.i] * fm * (I.rln + (E - 1.5f) * I.rlt) : 0.f;
   C.a8 = (mask & GK_T_VIII) ? ED * fm : 0.f;
 #pragma unroll
   for (int d = 0; d < 5; ++d) C.ws[d] = C.cI * P.dcoef[2][C.sg][d] + C.cDs * P.discoef[2][d];
@@ -365,7 +365,7 @@ gk_stage_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkStage
                     const int r = q / my, y = q - r * my;
                     const float2 gv = SW[r * ldy + y];
                     SG[(r0 + r) * ldy + y] = gv;
-                    gm.add(P, gv);
+                    gm.add(P, gv, P.ef[i]);
                   }
                 });
       }
@@ -465,7 +465,7 @@ gk_stage_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkStage
           nlv = SA[n * ldx + m];
         }
         return rhs_point<ST, decltype(modec)::value, decltype(intc)::value != 0>(
-            P, A, I, C, Q, slab, e, ip, m, pk, fmf, nlv, scale, fsum);
+            P, A, I, C, Q, slab, e, ip, m, pk, fmf, nlv, scale * P.ef[i], fsum);
       };
       auto epilogue = [&](auto modec, auto intc) {
         if constexpr (ROWMAP) {

@@ -116,6 +116,7 @@ __device__ __forceinline__ void ws_epilogue_role2(const GkDev &P, const GkStageA
     const float hx4 = (mask & GK_T_HYP) ? P.hyp_x * (P.invK * P.invK) * (P.invK * P.invK) : 0.f;
     const float hyp_m = (mask & GK_T_HYP) ? P.hyp_y * (P.invM * P.invM) * (P.invM * P.invM) * (fm2 * fm2) : 0.f;
     const float kap_m = fmf * kcz;
+    const float scale_i = scale * P.ef[i];   // ExB factor of this plane
     // parallel neighbours of this plane: uniform element offset + (wrap * kx shift) per thread
     const bool lowp = i < 2, seam = (i < 2) || (i >= P.ns - 2);
     int soff[4];
@@ -224,7 +225,7 @@ __device__ __forceinline__ void ws_epilogue_role2(const GkDev &P, const GkStageA
               // -i a z = a (z.y, -z.x)
               r = gkfft::caxpy(we.x * kap, make_float2(f0[q].y, -f0[q].x), r);
               r = gkfft::caxpy(we.y * fmf + we.z * kap, make_float2(chi0[q].y, -chi0[q].x), r);
-              r = gkfft::caxpy(scale, nlv[q], r);
+              r = gkfft::caxpy(scale_i, nlv[q], r);
               float2 out;
               if constexpr (MODE == 0) {
                 out = r;
@@ -439,6 +440,7 @@ gk_stage_ws2_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkS
     };
     // ---- Y2: inverse y pass 2, S -> dst (grad(chi) of the work item) ----
     GmaxAcc gm;
+    float ef_item = 1.f;   // ExB factor of the work item's plane
     auto y2_to = [&](float2 *dst) {
       for (int w = tid; w < MX_ * RY2; w += NTF) {
         const int r = w % MX_, k2 = w / MX_;
@@ -449,7 +451,7 @@ gk_stage_ws2_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkS
         dft<RY1, +1>(u);
         float2 *d = dst + r * LD + k2 * RY1;
 #pragma unroll
-        for (int k1 = 0; k1 < RY1; ++k1) { d[k1] = u[k1]; gm.add(P, u[k1]); }
+        for (int k1 = 0; k1 < RY1; ++k1) { d[k1] = u[k1]; gm.add(P, u[k1], ef_item); }
       }
     };
     // ---- YF: inverse y pass 2 of rows p and p + H, bracket d_y chi d_x f - d_x chi d_y f (real space
@@ -569,6 +571,7 @@ gk_stage_ws2_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkS
       // by the X1 of the previous slab, which every thread of the role has left)
       if (tid == 0) bulk_load(stg, (const ST *)A.y + (base0 + (long long)j0 * jstride), slab * sizeof(ST), mbar);
       float2 *chis = chis_cta + (it % GK_WS_CHI_RING) * 3 * slab;
+      ef_item = P.ef[i];
       build_chis(P, A, a, l, i, slab, NKY_, chis, tid, NTF);
       fsync();
       x1([&](int e) { return __ldcg(&chis[e]); });

@@ -250,6 +250,7 @@ gk_stage_ws4_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkS
     };
     // ---- Y2: inverse y pass 2, S -> SG (grad(chi) of the work item) ----
     GmaxAcc gm;
+    float ef_item = 1.f;   // ExB factor of the work item's plane
     auto y2_to_sg = [&]() {
       for (int w = tid; w < MQ * RY2; w += NTF) {
         const int r = w % MQ, k2 = w / MQ;
@@ -260,7 +261,7 @@ gk_stage_ws4_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkS
         dft<RY1, +1>(u);
         float2 *d = SG + r * LD + k2 * RY1;
 #pragma unroll
-        for (int k1 = 0; k1 < RY1; ++k1) { d[k1] = u[k1]; gm.add(P, u[k1]); }
+        for (int k1 = 0; k1 < RY1; ++k1) { d[k1] = u[k1]; gm.add(P, u[k1], ef_item); }
       }
     };
     // ---- YF: inverse y pass 2 of rows p and p + H, bracket d_y chi d_x f - d_x chi d_y f (real space
@@ -383,6 +384,7 @@ gk_stage_ws4_kernel(const __grid_constant__ GkDev P, const __grid_constant__ GkS
       const int l = al % P.nmu, a = al / P.nmu;
       const long long base0 = (((long long)a * P.nv * P.nmu + l) * P.ns + i) * P.slab;
       const int j0 = c * P.jchunk, j1 = min(P.nv, (c + 1) * P.jchunk);
+      ef_item = P.ef[i];
       // the first slab of the item lands while grad(chi) is built (the staging buffer was last read
       // by the X1 of the previous slab, which every thread of the role has left)
       if (tid == 0) bulk_load(stg, (const ST *)A.y + (base0 + (long long)j0 * jstride), slab * sizeof(ST), mbar);

@@ -68,10 +68,48 @@ inline void gauss_laguerre(int n, std::vector<double> &x, std::vector<double> &w
   }
 }
 
+// One point of the circular concentric (Lapillonne) model, PAPER.md:286-310 (reading R24), from gradient VECTORS in
+// the orthonormal frame (e_r, e_theta, e_phi) of the poloidal plane (R0 = 1: R = 1 + eps cos th, Z = eps sin th):
+// psi = eps, s = (th + eps sin th)/2pi, zeta = -phi/2pi + (q/pi) atan[sqrt((1-eps)/(1+eps)) tan(th/2)], q' = shat q/eps.
+struct CircPoint { double B, dBds, gpz, gzz, Dpsi, Dzeta, Epz, R, btfrac; };
+inline CircPoint circ_point(double q, double shat, double eps, double th) {
+  const double ct = std::cos(th), st = std::sin(th), R = 1.0 + eps * ct;
+  // zeta: chain rule through a = sqrt((1-eps)/(1+eps)), t = tan(th/2)
+  const double a = std::sqrt((1.0 - eps) / (1.0 + eps)), t = std::tan(0.5 * th), den = 1.0 + a * a * t * t;
+  const double A = std::atan(a * t);
+  const double dA_dth = a * 0.5 * (1.0 + t * t) / den;
+  const double dA_deps = t * (-1.0 / ((1.0 + eps) * (1.0 + eps) * a)) / den;
+  const double z_eps = (shat * q / eps) / kPi * A + q / kPi * dA_deps, z_th = q / kPi * dA_dth;
+  const double gpsi[3] = {1.0, 0.0, 0.0};
+  const double gs[3] = {st / (2.0 * kPi), R / (2.0 * kPi * eps), 0.0};
+  const double gz[3] = {z_eps, z_th / eps, -1.0 / (2.0 * kPi * R)};
+  auto dot = [](const double *x, const double *y) { return x[0] * y[0] + x[1] * y[1] + x[2] * y[2]; };
+  // B = delta / R (eq. 1) through its logarithmic derivatives; x = eps^2 / (q^2 (1 - eps^2))
+  const double x = eps * eps / (q * q * (1.0 - eps * eps));
+  const double dx = x * (2.0 / eps - 2.0 * shat / eps + 2.0 * eps / (1.0 - eps * eps));
+  const double delta = std::sqrt(1.0 + x), B = delta / R;
+  const double B_eps = B * (0.5 * dx / (1.0 + x) - ct / R), B_th = B * eps * st / R;
+  // derivatives at fixed (psi, s): the Jacobian of (eps, th) -> (psi, s) is [[1, 0], [s_eps, s_th]] (eq. 3)
+  const double s_eps = st / (2.0 * kPi), s_th = R / (2.0 * kPi);
+  const double dBds = B_th / s_th, dBdpsi = B_eps - s_eps * dBds;
+  const double gpp = dot(gpsi, gpsi), gpz = dot(gpsi, gz), gzz = dot(gz, gz), gps = dot(gpsi, gs), gzs = dot(gz, gs);
+  // E tensor: cofactors of the first two metric rows x pi dpf/dpsi / B^2; D from eq. 4
+  const double pref = kPi * (eps / (q * std::sqrt(1.0 - eps * eps))) / (B * B);
+  const double Epz = pref * (gpp * gzz - gpz * gpz), Eps = pref * (gpp * gzs - gps * gpz), Ezs = pref * (gpz * gzs - gps * gzz);
+  CircPoint c;
+  c.B = B; c.dBds = dBds; c.gpz = gpz; c.gzz = gzz;
+  c.Dpsi = -2.0 * Eps * dBds / B;
+  c.Dzeta = -2.0 * (-Epz * dBdpsi + Ezs * dBds) / B;
+  c.Epz = Epz; c.R = R; c.btfrac = 1.0 / delta;
+  return c;
+}
+
 struct Tables {
   int nsp, nv, nmu, ns, nkx, nky, K;
   double dkx, ds, dv, wv;
   std::vector<double> v, fmv, mu, wmu, fmm, B, F, BG, sth, cz, Rmaj, kx, ky, hypx, hypy;
+  std::vector<double> gpz, gzz, ef;   // k_perp^2 = kx^2 + 2 kx ky gpz + ky^2 gzz; ExB factor relative to ky/2
+  double kthnorm;
   std::vector<double> J0, G0, den, dinv, zinv;
   std::vector<double> vR;
   double dcoef[5][2][5], discoef[5][5];
@@ -85,7 +123,6 @@ inline void build_tables(const gk_grid &g, const gk_species *sp, const gk_salpha
   T.ds = 1.0 / ns;
   T.dv = 2.0 * g.vpar_max / nv;
   T.wv = T.dv;
-  T.dkx = 2.0 * kPi * geo.shat * g.ky0 / g.ikxspace;
   T.v.resize(nv); T.fmv.resize(nv);
   for (int j = 0; j < nv; ++j) {
     T.v[j] = -g.vpar_max + (j + 0.5) * T.dv;
@@ -104,6 +141,52 @@ inline void build_tables(const gk_grid &g, const gk_species *sp, const gk_salpha
       T.wmu[l] = vp * h;
     }
   }
+  // geometry: s-alpha (R2) or circular (R24)
+  T.B.resize(ns); T.F.resize(ns); T.BG.resize(ns); T.sth.resize(ns); T.cz.resize(ns); T.Rmaj.resize(ns);
+  T.gpz.resize(ns); T.gzz.resize(ns); T.ef.resize(ns);
+  T.fmm.resize((size_t)nmu * ns);
+  double kx_per_turn = 2.0 * kPi * geo.shat;      // kx gained per poloidal turn and unit ky
+  if (o.geometry == 0) {
+    T.kthnorm = geo.q / (2.0 * kPi * geo.eps);
+    for (int i = 0; i < ns; ++i) {
+      const double th = 2.0 * kPi * (-0.5 + (i + 0.5) * T.ds);
+      const double ct = std::cos(th), st = std::sin(th);
+      T.Rmaj[i] = 1.0 + geo.eps * ct;
+      T.B[i] = 1.0 / T.Rmaj[i];
+      T.F[i] = 0.5 / (kPi * geo.q);
+      T.BG[i] = geo.eps * st / (geo.q * T.Rmaj[i] * T.Rmaj[i]);
+      T.sth[i] = st;
+      T.cz[i] = ct + geo.shat * th * st;
+      T.gpz[i] = geo.shat * th;
+      T.gzz[i] = 1.0 + geo.shat * geo.shat * th * th;
+      T.ef[i] = 1.0;
+    }
+  } else {
+    T.kthnorm = std::sqrt(circ_point(geo.q, geo.shat, geo.eps, 0.0).gzz);
+    kx_per_turn = (geo.shat * geo.q / geo.eps) / T.kthnorm;   // g_psizeta grows by q' per turn of the branch-tracked arctan
+    const double b_ups = 1.0 / (2.0 * kPi * geo.q * std::sqrt(1.0 - geo.eps * geo.eps));
+    for (int i = 0; i < ns; ++i) {
+      const double sv = -0.5 + (i + 0.5) * T.ds;
+      double lo = 2.0 * kPi * sv - 1.0, hi = 2.0 * kPi * sv + 1.0;   // th + eps sin th = 2 pi s by bisection (monotone)
+      for (int it = 0; it < 200; ++it) {
+        const double mid = 0.5 * (lo + hi);
+        (mid + geo.eps * std::sin(mid) < 2.0 * kPi * sv ? lo : hi) = mid;
+      }
+      const CircPoint c = circ_point(geo.q, geo.shat, geo.eps, 0.5 * (lo + hi));
+      T.B[i] = c.B;
+      T.F[i] = b_ups / c.B;                                  // ffun
+      T.BG[i] = T.F[i] * c.dBds;                             // B gfun = F d_s B
+      T.sth[i] = -c.Dpsi;                                    // kappa = kx D^psi + (ky / kthnorm) D^zeta = -(kx sth + ky cz)
+      T.cz[i] = -c.Dzeta / T.kthnorm;
+      T.gpz[i] = c.gpz / T.kthnorm;
+      T.gzz[i] = c.gzz / (T.kthnorm * T.kthnorm);
+      T.ef[i] = 2.0 * c.Epz / T.kthnorm;                     // E^{psi zeta} k_zeta = ef ky / 2
+      T.Rmaj[i] = c.R * c.btfrac;                            // R B_t / B of the momentum flux (R18)
+    }
+  }
+  for (int i = 0; i < ns; ++i)
+    for (int l = 0; l < nmu; ++l) T.fmm[(size_t)l * ns + i] = std::exp(-2.0 * T.mu[l] * T.B[i]);
+  T.dkx = kx_per_turn * g.ky0 / g.ikxspace;
   T.kx.resize(nkx); T.ky.resize(nky); T.hypx.resize(nkx); T.hypy.resize(nky);
   for (int ip = 0; ip < nkx; ++ip) {
     T.kx[ip] = (ip - K) * T.dkx;
@@ -112,21 +195,6 @@ inline void build_tables(const gk_grid &g, const gk_species *sp, const gk_salpha
   for (int m = 0; m < nky; ++m) {
     T.ky[m] = m * g.ky0;
     T.hypy[m] = (nky > 1) ? o.disp_y * std::pow((double)m / (nky - 1), 4) : 0.0;
-  }
-  // s-alpha geometry (R2)
-  T.B.resize(ns); T.F.resize(ns); T.BG.resize(ns); T.sth.resize(ns); T.cz.resize(ns); T.Rmaj.resize(ns);
-  T.fmm.resize((size_t)nmu * ns);
-  std::vector<double> theta(ns);
-  for (int i = 0; i < ns; ++i) {
-    theta[i] = 2.0 * kPi * (-0.5 + (i + 0.5) * T.ds);
-    const double ct = std::cos(theta[i]), st = std::sin(theta[i]);
-    T.Rmaj[i] = 1.0 + geo.eps * ct;
-    T.B[i] = 1.0 / T.Rmaj[i];
-    T.F[i] = 0.5 / (kPi * geo.q);
-    T.BG[i] = geo.eps * st / (geo.q * T.Rmaj[i] * T.Rmaj[i]);
-    T.sth[i] = st;
-    T.cz[i] = ct + geo.shat * theta[i] * st;
-    for (int l = 0; l < nmu; ++l) T.fmm[(size_t)l * ns + i] = std::exp(-2.0 * T.mu[l] * T.B[i]);
   }
   // FLR kernels and Poisson denominators
   const size_t nphi = (size_t)ns * nkx * nky;
@@ -141,8 +209,8 @@ inline void build_tables(const gk_grid &g, const gk_species *sp, const gk_salpha
       for (int ip = 0; ip < nkx; ++ip)
         for (int m = 0; m < nky; ++m) {
           const size_t e = ((size_t)i * nkx + ip) * nky + m;
-          const double kxl = T.kx[ip] + geo.shat * theta[i] * T.ky[m];
-          const double kperp = std::sqrt(kxl * kxl + T.ky[m] * T.ky[m]);
+          const double kperp = std::sqrt(T.kx[ip] * T.kx[ip] + 2.0 * T.kx[ip] * T.ky[m] * T.gpz[i] +
+                                         T.ky[m] * T.ky[m] * T.gzz[i]);                                    // eq. 2
           const double arg = rho * kperp / T.B[i];
           const double g0 = bessel_i0e(0.5 * arg * arg);
           T.G0[(size_t)a * nphi + e] = g0;

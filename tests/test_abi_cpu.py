@@ -43,7 +43,7 @@ def test_no_cpu_fallback():
     g = binding._Grid(9, 4, 8, 8, 2, 0.1, 1, 4.0, 0, 3.0)
     sp = (binding._Species * 1)(binding._Species(1, 1, 1, 1, 7, 2))
     geo = binding._Salpha(1.5, 0.8, 0.18)
-    o = binding._Opts(1, 1, 1.0, 1.0, 1, 1.0, 0.2, 0.1, 0.1, 0, 0, 0, 0, 0)
+    o = binding._Opts(1, 1, 1.0, 1.0, 1, 1.0, 0.2, 0.1, 0.1, 0, 0, 0, 0, 0, 0)
     h = C.c_void_p()
     rc = lib.gk_create(C.byref(g), sp, C.byref(geo), C.byref(o), None, C.byref(h))
     assert rc == binding.GK_ECUDA
@@ -55,7 +55,7 @@ def test_gk_create_rejects_bad_arguments_before_touching_the_device():
     lib = binding.load_library()
     sp = (binding._Species * 1)(binding._Species(1, 1, 1, 1, 7, 2))
     geo = binding._Salpha(1.5, 0.8, 0.18)
-    o = binding._Opts(1, 1, 1.0, 1.0, 1, 1.0, 0.2, 0.1, 0.1, 0, 0, 0, 0, 0)
+    o = binding._Opts(1, 1, 1.0, 1.0, 1, 1.0, 0.2, 0.1, 0.1, 0, 0, 0, 0, 0, 0)
     h = C.c_void_p()
     for bad in [dict(nkx=8), dict(ns=3), dict(nvpar=3), dict(nky=0), dict(nmu=0), dict(ikxspace=0)]:
         kw = dict(nkx=9, nky=4, ns=8, nvpar=8, nmu=2, ky0=0.1, ikxspace=1, vpar_max=4.0, mu_grid=0, vperp_max=3.0)

@@ -259,3 +259,56 @@ def test_error_behaviour():
     assert g.lib.gk_rhs(g._h, C.c_void_p(fd.data_ptr()), None, None) == b.GK_EINVAL
     g.gk_rhs(fd)                                            # still usable after an EINVAL
     assert g.gk_launch_count() >= 4
+
+
+# ---- circular (Lapillonne) geometry, PAPER.md:286-310 (R24): gk_opts.geometry = 1 ---------------------------------
+def _circ(cfg):
+    cfg["opts"]["geometry"] = 1
+    cfg["geom"].update(q=1.4, shat=0.78, eps=0.19)
+    return cfg
+
+
+def test_circular_geometry_tables_match_the_oracles():
+    # the product builds its geometry from gradient vectors and logarithmic derivatives, the oracle from closed forms
+    cfg = _circ(small_cfg(**MID))
+    g, o = _ctx(cfg), GkRef(cfg)
+    for name in ("B", "F", "BG", "sth", "cz", "gpz", "gzz", "ef", "R", "kthnorm", "dkx", "kx", "J0", "Gamma0", "FM"):
+        np.testing.assert_allclose(g.gk_export_table(name), o.table(name).ravel(), rtol=1e-10, atol=1e-13, err_msg=name)
+
+
+@pytest.mark.parametrize("case", ["mid", "mid_kinetic", "mid_linear", "cfg3_plane", "cfg5_plane"])
+def test_circular_geometry_rhs_steps_fluxes_and_cfl(case):
+    import torch
+    kw = {"mid": MID, "mid_kinetic": dict(nspecies=2, adiabatic=0, **MID), "mid_linear": dict(nonlinear=0, **MID),
+          "cfg3_plane": dict(nkx=85, nky=32, ky0=0.035, ikxspace=5, ns=8, nvpar=8, nmu=2, mu_grid=1),
+          "cfg5_plane": dict(nkx=127, nky=64, ky0=0.0175, ikxspace=5, ns=8, nvpar=8, nmu=2, mu_grid=1)}[case]
+    cfg = _circ(small_cfg(**kw))
+    g = _ctx(cfg)
+    p = g.plan()
+    nl = bool(cfg["opts"]["nonlinear"])
+    o = GkRef(cfg, pad=(p["mx"], p["my"]) if nl else (0, 0))
+    f = rand_c(np.random.default_rng(91), o.shape, False).astype(np.complex64)
+    rhs, phi = g.gk_rhs(g.to_state(f))
+    ref, phiref = o.rhs(f)
+    assert rel_l2(phi.cpu().numpy(), phiref) < TOL_RHS
+    assert rel_l2(rhs.cpu().numpy(), ref) < TOL_RHS
+    est, eref = g.gk_estimate_dt(), o.estimate_dt(phi.cpu().numpy().astype(np.complex128))
+    for k in range(4):
+        if np.isinf(eref[k]):
+            assert np.isinf(est[k])
+        else:
+            np.testing.assert_allclose(est[k], eref[k], rtol=1e-5)
+    # a few RK4 steps with the flux triple folded into the first stage
+    amp, dt = (0.003, 0.0005) if "kinetic" in case else (0.03, 0.01)
+    f = (amp * rand_c(np.random.default_rng(92), o.shape, True)).astype(np.complex64)
+    g.gk_set_diagnostics(True)
+    fd = g.to_state(f)
+    g.gk_rk4_steps(fd, dt, 1)
+    fl = g.gk_fluxes_last()
+    np.testing.assert_allclose(fl[:, 1:], o.fluxes(f, o.field_solve(f))[:, 1:], rtol=3e-4, atol=1e-9)
+    g.gk_rk4_steps(fd, dt, 2)
+    torch.cuda.synchronize()
+    f0 = f.astype(np.complex128)
+    got, want = g.from_state(fd).astype(np.complex128), o.rk4_step(f0, dt, 3)
+    assert rel_l2(got, want) < TOL_RK10
+    assert rel_l2(got - f0, want - f0) < 3e-5
