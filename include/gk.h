@@ -106,8 +106,8 @@ int gk_rk4_steps(gk_ctx *ctx, void *f_dev, double dt, int nsteps);
  * f_dev, copies f_dev -> f_host_out, all asynchronous on the context stream in that order (truly asynchronous
  * only for pinned host memory; pageable memory makes the copies synchronous).  f_host_in / f_host_out: host,
  * same layout and storage type as f, may alias; f_dev: device scratch of the size of f, caller-owned.  Does
- * not synchronise at the end: synchronise the stream before reading f_host_out.  GK_EINVAL on null pointers
- * or a workspace too small for gk_rk4_step. */
+ * not synchronise at the end: synchronise the stream before reading f_host_out.  GK_EINVAL on null pointers,
+ * a misaligned f_dev or a workspace too small for gk_rk4_step, checked before the upload is queued. */
 int gk_rk4_step_host(gk_ctx *ctx, const void *f_host_in, void *f_host_out, void *f_dev, double dt);
 
 /* A batch of independent RK4 steps on HOST buffers, software-pipelined over two device buffers: the upload of
@@ -116,7 +116,9 @@ int gk_rk4_step_host(gk_ctx *ctx, const void *f_host_in, void *f_host_out, void 
  * uploads).  f_host_in[k] / f_host_out[k]: nbatch host pointers (pinned memory, layout and storage type of f; an
  * output must not alias the input of a LATER problem), f_dev0 / f_dev1: two device scratch arrays of the size of
  * f, caller-owned.  Every problem takes exactly the path of gk_rk4_step_host (same kernels, same result).
- * Synchronises all three streams before returning.  GK_EINVAL on null pointers or nbatch < 0. */
+ * Synchronises all three streams before returning.  Every pointer, the workspace size and the alignment of the
+ * device buffers are checked BEFORE anything is enqueued (GK_EINVAL, nothing in flight); a CUDA failure later drains
+ * the three streams before it is returned. */
 int gk_rk4_batch_host(gk_ctx *ctx, const void *const *f_host_in, void *const *f_host_out, int nbatch,
                       void *f_dev0, void *f_dev1, double dt);
 

@@ -589,6 +589,8 @@ int gk_rk4_step(gk_ctx *c, void *f, double dt) { return gk_rk4_steps(c, f, dt, 1
 int gk_rk4_step_host(gk_ctx *c, const void *f_host_in, void *f_host_out, void *f_dev, double dt) {
   if (int r = usable(c)) return r;
   if (!f_host_in || !f_host_out || !f_dev) return fail(c, GK_EINVAL, "gk_rk4_step_host: null pointer");
+  if (!c->ws || c->ws_bytes < c->need_full || ((uintptr_t)f_dev & 15))   // checked before the upload is queued
+    return fail(c, GK_EINVAL, "gk_rk4_step_host: workspace too small for gk_rk4_step or f_dev not 16-byte aligned");
   const size_t bytes = (size_t)c->P.ntot * c->elem_bytes;
   GK_CUDA(c, cudaMemcpyAsync(f_dev, f_host_in, bytes, cudaMemcpyHostToDevice, c->stream));
   if (int r = gk_rk4_steps(c, f_dev, dt, 1)) return r;
@@ -599,8 +601,13 @@ int gk_rk4_step_host(gk_ctx *c, const void *f_host_in, void *f_host_out, void *f
 int gk_rk4_batch_host(gk_ctx *c, const void *const *f_in, void *const *f_out, int nbatch, void *dev0, void *dev1,
                       double dt) {
   if (int r = usable(c)) return r;
+  // everything is validated BEFORE anything is enqueued: no copy is in flight when an argument error is returned
   if (!f_in || !f_out || !dev0 || !dev1 || dev0 == dev1 || nbatch < 0)
     return fail(c, GK_EINVAL, "gk_rk4_batch_host: bad arguments");
+  for (int k = 0; k < nbatch; ++k)
+    if (!f_in[k] || !f_out[k]) return fail(c, GK_EINVAL, "gk_rk4_batch_host: null host pointer");
+  if (!c->ws || c->ws_bytes < c->need_full) return fail(c, GK_EINVAL, "gk_rk4_batch_host: workspace too small for gk_rk4_step");
+  if (((uintptr_t)dev0 | (uintptr_t)dev1) & 15) return fail(c, GK_EINVAL, "gk_rk4_batch_host: device buffers must be 16-byte aligned");
   if (!c->s_up) {
     GK_CUDA(c, cudaStreamCreateWithFlags(&c->s_up, cudaStreamNonBlocking));
     GK_CUDA(c, cudaStreamCreateWithFlags(&c->s_down, cudaStreamNonBlocking));
@@ -612,22 +619,34 @@ int gk_rk4_batch_host(gk_ctx *c, const void *const *f_in, void *const *f_out, in
   }
   const size_t bytes = (size_t)c->P.ntot * c->elem_bytes;
   void *dev[2] = {dev0, dev1};
+  // a failure past this point (a CUDA error) leaves no copy in flight either: the three streams are drained first
+  auto drained = [&](int rc) {
+    cudaStreamSynchronize(c->s_up);
+    cudaStreamSynchronize(c->stream);
+    cudaStreamSynchronize(c->s_down);
+    return rc;
+  };
+#define GK_CUDA_D(call)                                                                                   \
+  do {                                                                                                    \
+    cudaError_t e_ = (call);                                                                              \
+    if (e_ != cudaSuccess) return drained(fail(c, GK_ECUDA, std::string(#call) + ": " + cudaGetErrorString(e_))); \
+  } while (0)
   // the copy streams start after whatever the caller queued on the context stream
-  GK_CUDA(c, cudaEventRecord(c->e_done[0], c->stream));
-  GK_CUDA(c, cudaStreamWaitEvent(c->s_up, c->e_done[0], 0));
+  GK_CUDA_D(cudaEventRecord(c->e_done[0], c->stream));
+  GK_CUDA_D(cudaStreamWaitEvent(c->s_up, c->e_done[0], 0));
   for (int k = 0; k < nbatch; ++k) {
     const int b = k & 1;
-    if (!f_in[k] || !f_out[k]) return fail(c, GK_EINVAL, "gk_rk4_batch_host: null host pointer");
-    if (k >= 2) GK_CUDA(c, cudaStreamWaitEvent(c->s_up, c->e_out[b], 0));   // buffer b has been downloaded
-    GK_CUDA(c, cudaMemcpyAsync(dev[b], f_in[k], bytes, cudaMemcpyHostToDevice, c->s_up));
-    GK_CUDA(c, cudaEventRecord(c->e_in[b], c->s_up));
-    GK_CUDA(c, cudaStreamWaitEvent(c->stream, c->e_in[b], 0));
-    if (int r = gk_rk4_steps(c, dev[b], dt, 1)) return r;
-    GK_CUDA(c, cudaEventRecord(c->e_done[b], c->stream));
-    GK_CUDA(c, cudaStreamWaitEvent(c->s_down, c->e_done[b], 0));
-    GK_CUDA(c, cudaMemcpyAsync(f_out[k], dev[b], bytes, cudaMemcpyDeviceToHost, c->s_down));
-    GK_CUDA(c, cudaEventRecord(c->e_out[b], c->s_down));
+    if (k >= 2) GK_CUDA_D(cudaStreamWaitEvent(c->s_up, c->e_out[b], 0));   // buffer b has been downloaded
+    GK_CUDA_D(cudaMemcpyAsync(dev[b], f_in[k], bytes, cudaMemcpyHostToDevice, c->s_up));
+    GK_CUDA_D(cudaEventRecord(c->e_in[b], c->s_up));
+    GK_CUDA_D(cudaStreamWaitEvent(c->stream, c->e_in[b], 0));
+    if (int r = gk_rk4_steps(c, dev[b], dt, 1)) return drained(r);
+    GK_CUDA_D(cudaEventRecord(c->e_done[b], c->stream));
+    GK_CUDA_D(cudaStreamWaitEvent(c->s_down, c->e_done[b], 0));
+    GK_CUDA_D(cudaMemcpyAsync(f_out[k], dev[b], bytes, cudaMemcpyDeviceToHost, c->s_down));
+    GK_CUDA_D(cudaEventRecord(c->e_out[b], c->s_down));
   }
+#undef GK_CUDA_D
   GK_CUDA(c, cudaStreamSynchronize(c->s_up));
   GK_CUDA(c, cudaStreamSynchronize(c->stream));
   GK_CUDA(c, cudaStreamSynchronize(c->s_down));
@@ -723,7 +742,8 @@ int gk_spectra(gk_ctx *c, const void *phi, double *kx_spec, double *ky_spec) {
   const int n = c->P.nkx + c->P.nky;
   gk::gk_spectra_kernel<<<n, 256, 0, c->stream>>>(c->P, (const float2 *)phi, c->d_spec);
   ++c->launches;
-  std::vector<double> h(n);
+  std::vector<double> h;
+  try { h.resize(n); } catch (const std::bad_alloc &) { return fail(c, GK_ENOMEM, "gk_spectra: out of host memory"); }
   cudaError_t e = cudaMemcpyAsync(h.data(), c->d_spec, n * sizeof(double), cudaMemcpyDeviceToHost, c->stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
   if (e != cudaSuccess) return fail(c, GK_ECUDA, std::string("gk_spectra: ") + cudaGetErrorString(e));

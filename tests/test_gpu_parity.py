@@ -259,6 +259,18 @@ def test_error_behaviour():
     assert g.lib.gk_rhs(g._h, C.c_void_p(fd.data_ptr()), None, None) == b.GK_EINVAL
     g.gk_rhs(fd)                                            # still usable after an EINVAL
     assert g.gk_launch_count() >= 4
+    # gk_rk4_batch_host validates every argument before it enqueues anything: a null pointer in the LAST
+    # problem leaves the outputs of the earlier ones untouched
+    import torch
+    g2 = _ctx(small_cfg(**MID))
+    hin = g2.to_state(gkinputs.initial_f(small_cfg(**MID))).cpu().pin_memory()
+    hout = torch.full_like(hin, 7.0).pin_memory()
+    d0, d1 = g2.empty_state(), g2.empty_state()
+    ins = (C.c_void_p * 2)(hin.data_ptr(), hin.data_ptr())
+    outs = (C.c_void_p * 2)(hout.data_ptr(), None)
+    rc = g2.lib.gk_rk4_batch_host(g2._h, ins, outs, 2, C.c_void_p(d0.data_ptr()), C.c_void_p(d1.data_ptr()), 0.01)
+    torch.cuda.synchronize()
+    assert rc == b.GK_EINVAL and bool((hout == 7.0).all())
 
 
 # ---- circular (Lapillonne) geometry, PAPER.md:286-310 (R24): gk_opts.geometry = 1 ---------------------------------
