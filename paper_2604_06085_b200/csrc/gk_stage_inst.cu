@@ -44,7 +44,8 @@ template <class ST> StagePick pick_stage(int mx, int my, int nky, int nkx, bool 
   if (nl && mx == MX && my == MY && nky == NKY && nkx == NKX)                     \
     return {(const void *)gk::gk_stage_ws4_kernel<ST, MX, MY, NKY, NKX, 4, NTF, NTE, RF, RE, NB>, NTF + NTE, GK_KIND_WS4, \
             gk::ws4_smem_bytes<ST, MX, MY, NKY, NKX, 4, NTE>(), 4, 1, gk::ws4_chis_elems<NKY, NKX, 4>(), GK_WS_NL_RING * slab}
-  GK_WS4(192, 192, 64, 127, 384, 256, 56, 152, 1);
+  // register split measured on B200 (ms per stage): 56/152 11.56, 64/144 11.45, 72/128 11.16, 80/120 11.59, 88/104 12.33
+  GK_WS4(192, 192, 64, 127, 384, 256, 72, 128, 1);
 #undef GK_WS4
   // term III off: streaming kernel (threads, shares per slab, vector items in flight)
 #define GK_LIN(NKY, NKX, NT, NSH, NB)                                             \
