@@ -178,7 +178,9 @@ def test_rk4_steps_parity_on_the_production_kernels(case):
 def _plane_cfg(base, ns=8, nvpar=8, nmu=2, **kw):
     from tests.util import small_cfg
     grid, kind = SPECIALISED[base]
-    return small_cfg(ns=ns, nvpar=nvpar, nmu=nmu, mu_grid=1, **grid, **kw), kind
+    args = dict(grid)
+    args.update(kw)                      # e.g. ky0 = 0.2 with kinetic electrons (R5)
+    return small_cfg(ns=ns, nvpar=nvpar, nmu=nmu, mu_grid=1, **args), kind
 
 
 @pytest.mark.parametrize("case", ["cfg2_plane", "cfg3_plane", "cfg5_plane", "cfg3_plane_linear", "cfg5_plane_linear"])
@@ -359,3 +361,30 @@ def test_two_contexts_of_different_generic_shapes_interleaved():
     ra1 = ga.gk_rhs(ga.to_state(fa))[0].cpu().numpy()
     assert np.array_equal(ra0, ra1)
     assert rel_l2(ra1, GkRef(big).rhs(fa)[0]) < 1e-5 and rel_l2(rb, GkRef(small).rhs(fb)[0]) < 1e-5
+
+
+@pytest.mark.parametrize("case", ["cfg3_plane", "cfg5_plane", "cfg3_plane_kinetic"])
+def test_ten_rk4_steps_on_the_production_planes(case):
+    # north_star: <= 1e-4 after 10 RK4 steps, on the kernels BASELINE configs 3, 4 and 5 run (their (kx, ky) planes at
+    # reduced depth along s, vpar, mu; config 2 takes the ten steps at full size above)
+    import torch
+    from paper_2604_06085_b200 import GkContext
+    from tests.util import rand_c
+    kin = case.endswith("_kinetic")
+    kw = dict(nspecies=2, adiabatic=0, ky0=0.2) if kin else {}
+    cfg, kind = _plane_cfg(case.replace("_kinetic", ""), **kw)
+    g, o = GkContext(cfg), GkRef(cfg)
+    assert g.plan()["kind"] == kind
+    amp, dt = (0.002, 0.0005) if kin else (0.01, 0.01)
+    if kin:     # the step the CFL estimate allows (field bound of the omega_H mode, R23), with a safety factor
+        est = o.estimate_dt(np.zeros(o.phi_shape, complex))
+        dt = 0.4 * min(est[2], est[3])
+    f = (rand_c(np.random.default_rng(78), o.shape, True) * amp).astype(np.complex64)
+    fd = g.to_state(f)
+    g.gk_rk4_steps(fd, dt, 10)
+    torch.cuda.synchronize()
+    f0 = f.astype(np.complex128)
+    got, ref = g.from_state(fd).astype(np.complex128), o.rk4_step(f0, dt, 10)
+    assert np.isfinite(ref).all() and np.abs(ref).max() < 10 * np.abs(f0).max()
+    assert rel_l2(got, ref) < 1e-4
+    assert rel_l2(got - f0, ref - f0) < 1e-4, rel_l2(got - f0, ref - f0)
