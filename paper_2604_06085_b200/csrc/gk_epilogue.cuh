@@ -142,9 +142,12 @@ __device__ __forceinline__ void epi_item(const GkDev &P, const GkStageArgs &A, H
   constexpr int PV = M::PV, RS = M::RS, EPT = M::EPT, KS = M::KS;
   constexpr bool NL = H::NL;
   const int m0 = (et % M::VPR) * PV, r0 = et / M::VPR;
-  const int el0 = r0 * nky + m0;              // index of item 0 inside the share
+  // a thread whose first row lies beyond a short share (r0 >= nrows: it has no valid item at all) addresses row 0 of
+  // the share instead: every address it forms stays inside the slab, and nothing it computes is stored
+  const int r0a = r0 < nrows ? r0 : 0;
+  const int el0 = r0a * nky + m0;             // index of item 0 inside the share
   const int e0 = row0 * nky + el0;            // ... inside the slab
-  const int ip0 = row0 + r0;                  // kx row of item 0
+  const int ip0 = row0 + r0a;                 // kx row of item 0
   const float scale = 0.25f * P.ef[i] * P.fftnorm;      // ef/2 (bracket) * 1/2 (two-for-one unpack) / (mx my)
   const long long jstride = (long long)P.nmu * P.ns * P.slab;
   const int js = (int)jstride;

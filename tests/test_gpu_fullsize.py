@@ -278,7 +278,8 @@ def test_config3_gradient_scan_on_the_production_kernel(rlt):
     assert rel_l2(GkRef(cfg7).rk4_step(f0, 0.01, 1) - f0, o.rk4_step(f0, 0.01, 1) - f0) > 3e-3
 
 
-@pytest.mark.parametrize("case", ["cfg3_plane_bf16", "cfg5_plane_bf16", "cfg3_plane_linear_f16"])
+@pytest.mark.parametrize("case", ["cfg3_plane_bf16", "cfg5_plane_bf16", "cfg3_plane_linear_f16", "cfg2_plane_linear_f16",
+                                  "cfg5_plane_linear_bf16"])
 def test_half_storage_on_the_production_kernels(case):
     import torch
     from paper_2604_06085_b200 import GkContext
