@@ -162,6 +162,31 @@ int gk_rk4_steps_cfl(gk_ctx *ctx, void *f_dev, int nsteps, double safety, double
  * deterministic (one block tree per output, no atomics).  Synchronises the stream.  GK_EINVAL on null. */
 int gk_spectra(gk_ctx *ctx, const void *phi_dev, double *kx_spec_host, double *ky_spec_host);
 
+/* gk_spectra for callers that cannot allocate device memory.  gk_spectra needs a context, and gk_create builds one
+ * out of cudaMalloc'ed tables; that rules it out for a host whose own pool allocator already owns the whole device
+ * (every further cudaMalloc fails), for a process under an MPS / MIG memory cap, and for a loop that cannot take
+ * cudaMalloc's device-wide synchronisation.  This entry point needs no context and calls no cudaMalloc, cudaFree or
+ * allocating library routine: the caller passes the input and the outputs, and the nkx + nky device-side results
+ * are staged in a fixed array inside the library image (GK_SPECTRA_STATIC_MAX doubles = 32 KiB, held by every GPU
+ * that loads libgk.so until the process exits).
+ *   phi_dev:       device, [ns][nkx][nky] complex64, on the CURRENT device;
+ *   kx_spec_host:  host, nkx doubles;  ky_spec_host: host, nky doubles -- same definition, normalisation and
+ *                  summation order as gk_spectra (the results are bit-identical);
+ *   cuda_stream:   a cudaStream_t of the current device cast to void*, NULL = default stream.
+ * Limit: nkx + nky <= GK_SPECTRA_STATIC_MAX, else GK_EINVAL (nothing is launched); also GK_EINVAL for null pointers
+ * and sizes < 1, GK_ECUDA for CUDA failures.  The text of the last error of the calling thread is returned by
+ * gk_spectra_static_error() ("" after a successful call).
+ * Set-up: the first call on each device resolves that device's address of the array (cudaGetSymbolAddress); make
+ * that first call with the device current and before any stream capture begins.
+ * Sharing: all calls on a device use the same array, which keeps the previous call's numbers.  Each call overwrites
+ * exactly the entries it reads back, so nothing needs clearing -- but two calls that overlap on the GPU (two
+ * streams, or two host threads) race on it: serialise them.  Launches one kernel, then synchronises the stream. */
+#define GK_SPECTRA_STATIC_MAX 4096
+int gk_spectra_static(const void *phi_dev, int ns, int nkx, int nky, double *kx_spec_host, double *ky_spec_host,
+                      void *cuda_stream);
+size_t gk_spectra_static_max(void);          /* GK_SPECTRA_STATIC_MAX of the library that was loaded */
+const char *gk_spectra_static_error(void);   /* never NULL; thread-local */
+
 /* Test hook: copies a create-time table to host memory as doubles.  `which` is one of
  * "vpar","mu","wmu","kx","ky","B","F","BG","J0","Gamma0","FM","den","zonal","pad","ef","gpz","gzz","sth","cz","R",
  * "kthnorm","dkx".  Returns the

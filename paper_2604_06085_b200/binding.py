@@ -90,6 +90,11 @@ def load_library(build_if_missing: bool = True):
     lib.gk_rk4_step_host.argtypes = [vp, vp, vp, vp, C.c_double]
     lib.gk_rk4_batch_host.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.c_int, vp, vp, C.c_double]
     lib.gk_spectra.argtypes = [vp, vp, dp, dp]
+    lib.gk_spectra_static.argtypes = [vp, C.c_int, C.c_int, C.c_int, dp, dp, vp]
+    lib.gk_spectra_static_max.restype = C.c_size_t
+    lib.gk_spectra_static_max.argtypes = []
+    lib.gk_spectra_static_error.restype = C.c_char_p
+    lib.gk_spectra_static_error.argtypes = []
     lib.gk_set_diagnostics.argtypes = [vp, C.c_int]
     lib.gk_fluxes_last.argtypes = [vp, dp]
     lib.gk_estimate_dt.argtypes = [vp, dp]
@@ -105,6 +110,32 @@ def load_library(build_if_missing: bool = True):
     lib.gk_version.restype = C.c_char_p
     _lib = lib
     return lib
+
+
+def gk_spectra_static(phi, stream=None):
+    """(kx_spec[nkx], ky_spec[nky]) of |phi|^2 without a context and without any device allocation: for hosts of
+    this library whose device memory is already fully claimed by another allocator, or capped, so that gk_create's
+    cudaMalloc calls cannot succeed.  `phi`: contiguous CUDA complex64 tensor [ns, nkx, nky] on the current device;
+    nkx + nky <= gk_spectra_static_max().  The device-side staging array is shared by every call: do not overlap
+    calls.  Same numbers as GkContext.gk_spectra."""
+    import numpy as np
+    import torch
+    lib = load_library()
+    if not (phi.is_cuda and phi.dtype == torch.complex64 and phi.is_contiguous() and phi.dim() == 3):
+        raise ValueError("phi: expected a contiguous CUDA complex64 tensor [ns, nkx, nky]")
+    ns, nkx, nky = (int(n) for n in phi.shape)
+    kxs, kys = np.zeros(nkx, np.float64), np.zeros(nky, np.float64)
+    st = stream if stream is not None else torch.cuda.current_stream(phi.device)
+    with torch.cuda.device(phi.device):
+        rc = lib.gk_spectra_static(C.c_void_p(phi.data_ptr()), ns, nkx, nky, kxs.ctypes.data_as(C.POINTER(C.c_double)),
+                                   kys.ctypes.data_as(C.POINTER(C.c_double)), C.c_void_p(st.cuda_stream))
+    if rc != GK_OK:
+        raise GkError(rc, lib.gk_spectra_static_error().decode())
+    return kxs, kys
+
+
+def gk_spectra_static_max() -> int:
+    return int(load_library().gk_spectra_static_max())
 
 
 _STORAGE = {"complex64": 0, "fp16": 1, "bf16": 2, 0: 0, 1: 1, 2: 2}

@@ -17,6 +17,7 @@ OBJDIR = os.path.join(HERE, "build")
 # its own translation unit so that the units compile in parallel
 UNITS = [
     ("gk_lib.cu", [], "gk_lib.o"),
+    ("gk_noalloc.cu", [], "gk_noalloc.o"),   # gk_spectra_static: context-free, fixed scratch in the library image
     ("gk_stage_inst.cu", ["-DGK_ST_ID=0"], "gk_stage_c64.o"),
     ("gk_stage_inst.cu", ["-DGK_ST_ID=1"], "gk_stage_f16.o"),
     ("gk_stage_inst.cu", ["-DGK_ST_ID=2"], "gk_stage_bf16.o"),
@@ -67,7 +68,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     from concurrent.futures import ThreadPoolExecutor
     os.makedirs(OBJDIR, exist_ok=True)
     fast = bool(os.environ.get("GK_FAST_BUILD"))           # developer builds only: complex64 storage
-    units = UNITS[:2] if fast else UNITS
+    units = UNITS[:3] if fast else UNITS
     extra = ["-DGK_ONLY_C64"] if fast else []
 
     flagfile = os.path.join(OBJDIR, "flags.txt")
