@@ -43,14 +43,28 @@ def _peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
+def _running_src_hash():
+    """The csrc/ hash compiled into the loaded library (gk_version "... src:<hash>")."""
+    from paper_2604_06085_b200 import load_library
+    v = load_library().gk_version().decode()
+    return v.rsplit("src:", 1)[1].strip() if "src:" in v else None
+
+
 def _ncu_record(workload):
     """Per-launch counters of the stage kernel from the committed ncu capture (profiles/stage_traffic.json):
-    {"dram_gb": ..., "l1_wavefronts": ...} or None if this workload was not captured."""
+    ({"dram_gb": ..., "l1_wavefronts": ...} or None if this workload was not captured, stale).  A record belongs to
+    the csrc/ tree it was captured from (`src_hash`); if the running library was built from another tree the
+    counters are NOT quoted: (None, True)."""
     p = os.path.join(ROOT, "profiles", "stage_traffic.json")
-    if os.path.exists(p):
-        with open(p) as fh:
-            return json.load(fh).get(workload)
-    return None
+    if not os.path.exists(p):
+        return None, False
+    with open(p) as fh:
+        rec = json.load(fh).get(workload)
+    if rec is None:
+        return None, False
+    if rec.get("src_hash") is None or rec.get("src_hash") != _running_src_hash():
+        return None, True
+    return rec, False
 
 
 SM_COUNT, FP32_LANES, SM_MAX_MHZ = 148, 128, 1965.0      # B200 (B200_PROFILING.md)
@@ -79,13 +93,14 @@ def stage_rooflines(cfg, plan, npts, storage, stage_avg_ms, sm_mhz, nonlinear):
     t = stage_avg_ms * 1e-3
     achieved = bpp * npts / t / 1e9
     key = cfg["name"] + ("" if nonlinear else "+linear") + ("" if storage == 0 else "+half")
-    rec = _ncu_record(key) or {}
+    rec, stale = _ncu_record(key)
+    rec = rec or {}
     clock = (sm_mhz or SM_MAX_MHZ) * 1e6
     fpp = fp32_flops_per_point(cfg["grid"], plan, nonlinear)
     fp32_peak = SM_COUNT * FP32_LANES * 2 * SM_MAX_MHZ * 1e6 / 1e12
     fp32 = fpp * npts / t / 1e12
     out = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-           "traffic": rec.get("dram_gb"),
+           "traffic": rec.get("dram_gb"), "traffic_stale": stale, "traffic_kernel": rec.get("kernel"),
            "traffic_unit": "GB of DRAM read+write per stage-kernel launch (ncu --set full, profiles/)",
            "peak_source": peak_src, "avg_launch_ms": stage_avg_ms, "alg_bytes_per_point": bpp,
            "fp32": {"bound": "alu", "achieved": fp32, "peak": fp32_peak, "unit": "TFLOP/s", "frac": fp32 / fp32_peak,

@@ -139,7 +139,8 @@ int gk_fluxes_last(gk_ctx *ctx, double *out_host);
 /* CFL estimate of the time step (PAPER.md:340 estimate_timestep; readings R21-R23).  out_host[4]:
  *   [1] nonlinear bound 2 sqrt2 / max (1/2)(|d_y chi| kx_max + |d_x chi| ky_max), the maximum taken over the padded
  *       real-space grad(chi) of every (species, mu, s) as built by the MOST RECENT stage launch (gk_rhs or the last
- *       stage of gk_rk4_step(s): "one-step lag"); +inf before the first launch, for phi = 0 and with term III off;
+ *       stage of gk_rk4_step(s): "one-step lag"; a bare gk_field_solve leaves it as it is); +inf before the first
+ *       launch, after gk_reset_cfl, for phi = 0 and with term III off;
  *   [2] von Neumann bound of the streaming and trapping stencils with their dissipation (create-time);
  *   [3] field (omega_H) bound with kinetic electrons, +inf with adiabatic electrons (create-time);
  *   [0] the minimum of the three.
@@ -153,6 +154,12 @@ int gk_estimate_dt(gk_ctx *ctx, double *out_host);
  * (one double) may be NULL.  Synchronises once per step. */
 int gk_rk4_steps_cfl(gk_ctx *ctx, void *f_dev, int nsteps, double safety, double dt_max, double *dt_used_host,
                      double *t_advanced_host);
+/* The nonlinear bound lives in the context and belongs to whatever state the last stage launch saw.  A context that
+ * is reused for another state (a new initial condition, or after gk_rhs on some other f) therefore starts
+ * gk_rk4_steps_cfl / gk_estimate_dt from that unrelated bound.  gk_reset_cfl puts the context back to "no stage
+ * launched yet" ([1] = +inf, so the first step uses the linear-only estimate); asynchronous on the
+ * context stream.  gk_field_solve on its own never changes the bound. */
+int gk_reset_cfl(gk_ctx *ctx);
 
 /* Spectra of the potential (ky_spec = sum_{s,kx} |phi|^2, kx_spec = sum_{s,ky} |phi|^2, with the
  * Parseval factor P_ky (1 at ky = 0, 2 otherwise) and the weight Delta s = 1/ns applied; R20):
@@ -194,7 +201,8 @@ const char *gk_spectra_static_error(void);   /* never NULL; thread-local */
 size_t gk_export_table(const gk_ctx *ctx, const char *which, double *host_out, size_t max_doubles);
 
 const char *gk_last_error(const gk_ctx *ctx); /* never NULL; "" if no error */
-const char *gk_version(void);
+const char *gk_version(void);  /* "gk-b200 <ver> (sm_100a) src:<16 hex digits>": the digits identify the csrc/ tree the
+                                  library was built from (paper_2604_06085_b200/build.py src_hash) */
 
 #ifdef __cplusplus
 }

@@ -98,6 +98,7 @@ def load_library(build_if_missing: bool = True):
     lib.gk_set_diagnostics.argtypes = [vp, C.c_int]
     lib.gk_fluxes_last.argtypes = [vp, dp]
     lib.gk_estimate_dt.argtypes = [vp, dp]
+    lib.gk_reset_cfl.argtypes = [vp]
     lib.gk_rk4_steps_cfl.argtypes = [vp, vp, C.c_int, C.c_double, C.c_double, dp, dp]
     lib.gk_export_table.restype = C.c_size_t
     lib.gk_export_table.argtypes = [vp, C.c_char_p, dp, C.c_size_t]
@@ -309,6 +310,10 @@ class GkContext:
         out = np.zeros(4, np.float64)
         self._check(self.lib.gk_estimate_dt(self._h, out.ctypes.data_as(C.POINTER(C.c_double))))
         return out
+
+    def gk_reset_cfl(self):
+        """Forget the nonlinear CFL bound of the last stage launch (context reused for another state)."""
+        self._check(self.lib.gk_reset_cfl(self._h))
 
     def gk_rk4_steps_cfl(self, f, nsteps, safety, dt_max=0.0):
         """CFL-adaptive steps; returns (dt of every step, time advanced)."""

@@ -42,6 +42,18 @@ def _nvcc() -> str:
     return "nvcc"
 
 
+def src_hash() -> str:
+    """sha256 (16 hex digits) over the names and contents of every file of csrc/: compiled into gk_version() so that
+    counters captured from one build (profiles/stage_traffic.json) are never quoted for another."""
+    import hashlib
+    h = hashlib.sha256()
+    for path in _csrc_files():
+        h.update(os.path.basename(path).encode() + b"\0")
+        with open(path, "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()[:16]
+
+
 def _flags_now() -> str:
     fast = bool(os.environ.get("GK_FAST_BUILD"))           # developer builds only: complex64 storage
     return " ".join([*NVCC_FLAGS, *(["-DGK_ONLY_C64"] if fast else [])])
@@ -78,6 +90,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     def compile_unit(u):
         src, defs, obj = u
         objp = os.path.join(OBJDIR, obj)
+        if src == "gk_lib.cu":
+            defs = [*defs, f'-DGK_SRC_HASH="{src_hash()}"']
         cmd = [_nvcc(), *NVCC_FLAGS, *extra, *defs, "-c", os.path.join(CSRC, src), "-o", objp]
         deps = _csrc_files() + _include_files()
         if not force and same_flags and os.path.exists(objp) and all(os.path.getmtime(d) <= os.path.getmtime(objp) for d in deps):

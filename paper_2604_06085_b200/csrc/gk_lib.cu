@@ -198,9 +198,11 @@ void stage_launch(gk_ctx *c, const GkStageArgs &A) {
   }
 }
 
-int solve_phi_from_planes(gk_ctx *c, float2 *mom, float2 *phi) {
+// `gmax`: the CFL maximum to clear for the stage launch that follows this field solve (GmaxAcc), or nullptr if
+// none follows (the public gk_field_solve: the bound of the most recent stage launch must survive it).
+int solve_phi_from_planes(gk_ctx *c, float2 *mom, float2 *phi, unsigned int *gmax) {
   const GkDev &P = c->P;
-  gk::gk_phi_kernel<<<(unsigned)((P.nphi + 255) / 256), 256, 0, c->stream>>>(P, mom, phi, c->d_gmax);
+  gk::gk_phi_kernel<<<(unsigned)((P.nphi + 255) / 256), 256, 0, c->stream>>>(P, mom, phi, gmax);
   ++c->launches;
   if (P.adiabatic) {
     gk::gk_zonal_kernel<<<P.nkx, 32, 0, c->stream>>>(P, phi);
@@ -219,7 +221,11 @@ int usable(gk_ctx *c) {
 
 extern "C" {
 
-const char *gk_version(void) { return "gk-b200 0.1 (sm_100a)"; }
+#ifndef GK_SRC_HASH
+#define GK_SRC_HASH "unknown"
+#endif
+// "src:<hash>" = build.py's src_hash() of csrc/ at compile time (bench.py matches ncu captures against it)
+const char *gk_version(void) { return "gk-b200 0.1 (sm_100a) src:" GK_SRC_HASH; }
 
 const char *gk_last_error(const gk_ctx *c) { return c ? c->err.c_str() : "null context"; }
 
@@ -446,18 +452,29 @@ int create_impl(const gk_grid *g, const gk_species *sp, const gk_salpha *geo, co
 
 }  // namespace
 
-// No exception crosses the ABI: allocation failures of the host-side tables map to GK_ENOMEM, anything else
-// to GK_EINVAL (the context, if it was created, carries the text).
-#define GK_GUARDED(ctx, expr)                                                     \
-  try {                                                                           \
-    return (expr);                                                                \
-  } catch (const std::bad_alloc &) {                                              \
-    return fail(ctx, GK_ENOMEM, "out of host memory");                            \
-  } catch (const std::exception &e) {                                             \
-    return fail(ctx, GK_EINVAL, std::string("internal error: ") + e.what());      \
-  } catch (...) {                                                                 \
-    return fail(ctx, GK_EINVAL, "internal error");                                \
+// No exception crosses the ABI: an allocation failure of host-side containers maps to GK_ENOMEM, anything else to
+// GK_EINVAL.  The context, if there is one, is poisoned (it may be half-built or half-updated) and carries the text
+// where that text can still be stored.
+namespace {
+int caught(gk_ctx *c, int code, const char *what) noexcept {
+  if (c) {
+    c->poisoned = true;
+    try { c->err = what; } catch (...) {}
   }
+  return code;
+}
+template <class F> int guarded(gk_ctx *c, F &&body) noexcept {
+  try {
+    return body();
+  } catch (const std::bad_alloc &) {
+    return caught(c, GK_ENOMEM, "out of host memory");
+  } catch (const std::exception &e) {
+    return caught(c, GK_EINVAL, e.what());
+  } catch (...) {
+    return caught(c, GK_EINVAL, "internal error");
+  }
+}
+}  // namespace
 
 extern "C" {
 
@@ -465,10 +482,12 @@ int gk_create(const gk_grid *g, const gk_species *sp, const gk_salpha *geo, cons
               void *cuda_stream, gk_ctx **out) {
   try {
     return create_impl(g, sp, geo, o, cuda_stream, out);
-  } catch (const std::bad_alloc &) {
-    return GK_ENOMEM;
+  } catch (const std::bad_alloc &) {   // *out, if set, is half-built: unusable from here on, caller destroys it
+    return caught(out ? *out : nullptr, GK_ENOMEM, "gk_create: out of host memory");
+  } catch (const std::exception &e) {
+    return caught(out ? *out : nullptr, GK_EINVAL, e.what());
   } catch (...) {
-    return GK_EINVAL;
+    return caught(out ? *out : nullptr, GK_EINVAL, "gk_create: internal error");
   }
 }
 
@@ -496,21 +515,32 @@ int gk_set_workspace(gk_ctx *c, void *dev, size_t bytes) {
   return GK_OK;
 }
 
-int gk_field_solve(gk_ctx *c, const void *f, void *phi) {
+}  // extern "C"
+
+namespace {
+int field_solve(gk_ctx *c, const void *f, void *phi, unsigned int *gmax) {
   if (int r = usable(c)) return r;
   if (!f || !phi || !c->ws) return fail(c, GK_EINVAL, "gk_field_solve: null pointer or no workspace");
   float2 *mom = (float2 *)((char *)c->ws + c->off_mom);
 #define GK_CALL(ST) launch_moment<ST>(c, f, mom)
   GK_BY_STORAGE(c, GK_CALL);
 #undef GK_CALL
-  return solve_phi_from_planes(c, mom, (float2 *)phi);
+  return solve_phi_from_planes(c, mom, (float2 *)phi, gmax);
 }
+}  // namespace
+
+extern "C" {
+
+// A field solve on its own is followed by no stage launch: it leaves the CFL maximum of the last one alone, so
+// that step -> gk_field_solve (for gk_spectra / gk_fluxes) -> gk_estimate_dt still sees the nonlinear bound.
+int gk_field_solve(gk_ctx *c, const void *f, void *phi) { return field_solve(c, f, phi, nullptr); }
 
 int gk_rhs(gk_ctx *c, const void *f, void *phi, void *rhs) {
+  return guarded(c, [&]() -> int {
   if (int r = usable(c)) return r;
   if (!f || !phi || !rhs || rhs == f || !c->ws) return fail(c, GK_EINVAL, "gk_rhs: bad pointers or no workspace");
   if (((uintptr_t)f | (uintptr_t)rhs) & 15) return fail(c, GK_EINVAL, "gk_rhs: f and rhs must be 16-byte aligned");
-  if (int r = gk_field_solve(c, f, phi)) return r;
+  if (int r = field_solve(c, f, phi, c->d_gmax)) return r;
   GkStageArgs A;
   std::memset(&A, 0, sizeof(A));
   A.y = f; A.out = rhs; A.phi = (const float2 *)phi; A.mode = 0;
@@ -521,9 +551,11 @@ int gk_rhs(gk_ctx *c, const void *f, void *phi, void *rhs) {
   A.gmax = c->d_gmax;
   stage_launch(c, A);
   return check_launch(c, "stage kernel");
+  });
 }
 
 int gk_rk4_steps(gk_ctx *c, void *f, double dt, int nsteps) {
+  return guarded(c, [&]() -> int {
   if (int r = usable(c)) return r;
   if (!f || !c->ws || nsteps < 0) return fail(c, GK_EINVAL, "gk_rk4_steps: bad arguments or no workspace");
   if ((uintptr_t)f & 15) return fail(c, GK_EINVAL, "gk_rk4_steps: f must be 16-byte aligned (bulk copies of whole slabs)");
@@ -549,7 +581,7 @@ int gk_rk4_steps(gk_ctx *c, void *f, double dt, int nsteps) {
 #undef GK_CALL
     }
     // classical RK4: acc = f + dt/6 k1, then += dt/3 k2, += dt/3 k3, f = acc + dt/6 k4
-    if (int r = solve_phi_from_planes(c, mom, phi)) return r;
+    if (int r = solve_phi_from_planes(c, mom, phi, c->d_gmax)) return r;
     A.mode = 1; A.y = f; A.fn = f; A.out = ya; A.c = 0.5f * h; A.b = h / 6.f;
     const bool fused_diag = c->diag && c->stage_kind != GK_KIND_POINT && c->stage_kind != GK_KIND_LIN;
     if (c->diag && !fused_diag) {   // point kernel: no streaming role; streaming kernel: no registers to spare
@@ -570,18 +602,19 @@ int gk_rk4_steps(gk_ctx *c, void *f, double dt, int nsteps) {
       ++c->launches;
       c->flux_valid = true;
     }
-    if (int r = solve_phi_from_planes(c, mom, phi)) return r;
+    if (int r = solve_phi_from_planes(c, mom, phi, c->d_gmax)) return r;
     A.mode = 2; A.y = ya; A.fn = f; A.out = yb; A.c = 0.5f * h; A.b = h / 3.f;
     stage_launch(c, A);
-    if (int r = solve_phi_from_planes(c, mom, phi)) return r;
+    if (int r = solve_phi_from_planes(c, mom, phi, c->d_gmax)) return r;
     A.mode = 2; A.y = yb; A.fn = f; A.out = ya; A.c = h; A.b = h / 3.f;
     stage_launch(c, A);
-    if (int r = solve_phi_from_planes(c, mom, phi)) return r;
+    if (int r = solve_phi_from_planes(c, mom, phi, c->d_gmax)) return r;
     A.mode = 3; A.y = ya; A.fn = f; A.out = f; A.c = 0.f; A.b = h / 6.f;
     stage_launch(c, A);
     if (int r = check_launch(c, "stage kernel")) return r;
   }
   return GK_OK;
+  });
 }
 
 int gk_rk4_step(gk_ctx *c, void *f, double dt) { return gk_rk4_steps(c, f, dt, 1); }
@@ -715,6 +748,12 @@ int gk_estimate_dt(gk_ctx *c, double *out_host) {
   return GK_OK;
 }
 
+int gk_reset_cfl(gk_ctx *c) {
+  if (int r = usable(c)) return r;
+  GK_CUDA(c, cudaMemsetAsync(c->d_gmax, 0, sizeof(unsigned int), c->stream));
+  return GK_OK;
+}
+
 int gk_rk4_steps_cfl(gk_ctx *c, void *f, int nsteps, double safety, double dt_max, double *dt_used_host,
                      double *t_advanced_host) {
   if (int r = usable(c)) return r;
@@ -754,6 +793,7 @@ int gk_spectra(gk_ctx *c, const void *phi, double *kx_spec, double *ky_spec) {
 
 size_t gk_export_table(const gk_ctx *c, const char *which, double *out, size_t maxn) {
   if (!c || !which) return 0;
+  try {
   const gkt::Tables &T = c->T;
   const std::string w(which);
   std::vector<double> tmp;
@@ -780,6 +820,9 @@ size_t gk_export_table(const gk_ctx *c, const char *which, double *out, size_t m
   } else return 0;
   if (out) std::memcpy(out, src->data(), std::min(maxn, src->size()) * sizeof(double));
   return src->size();
+  } catch (...) {   // host allocation failure of a temporary: reported as "no such table"
+    return 0;
+  }
 }
 
 long long gk_launch_count(const gk_ctx *c) { return c ? c->launches : 0; }

@@ -20,6 +20,8 @@ PLANES = {
     "cfg5_plane": (dict(nkx=127, nky=64, ky0=0.0175, ikxspace=5, ns=8, nvpar=8, nmu=2, mu_grid=1), 5),
     "cfg3_plane_linear": (dict(nkx=85, nky=32, ky0=0.035, ikxspace=5, ns=8, nvpar=8, nmu=2, mu_grid=1, nonlinear=0), 3),
     "cfg5_plane_linear": (dict(nkx=127, nky=64, ky0=0.0175, ikxspace=5, ns=8, nvpar=8, nmu=2, mu_grid=1, nonlinear=0), 3),
+    # tiny plane without term III: the point kernel, whose fluxes come from the separate gk_flux_kernel pass
+    "tiny_linear": (dict(nkx=9, nky=4, ns=8, nvpar=8, nmu=2, nonlinear=0), 6),
 }
 
 
@@ -28,11 +30,12 @@ def _ctx(case, **kw):
     grid, kind = PLANES[case]
     cfg = small_cfg(**grid)
     g = GkContext(cfg, **kw)
-    assert g.plan()["kind"] == kind or (kind == 3 and g.plan()["kind"] == 7), g.plan()   # 3 / 7: linear kernels
+    assert g.plan()["kind"] == kind, g.plan()
     return cfg, g
 
 
-@pytest.mark.parametrize("case", ["mid", "mid_kinetic", "cfg2_plane", "cfg3_plane", "cfg5_plane", "cfg3_plane_linear"])
+@pytest.mark.parametrize("case", ["mid", "mid_kinetic", "cfg2_plane", "cfg3_plane", "cfg5_plane", "cfg3_plane_linear",
+                                  "tiny_linear"])
 def test_estimate_dt_parity(case):
     cfg, g = _ctx(case, full_workspace=False)
     p = g.plan()
@@ -59,6 +62,28 @@ def test_estimate_dt_parity(case):
     if nl:
         g.gk_rhs(g.to_state(0.25 * f))
         np.testing.assert_allclose(g.gk_estimate_dt()[1], 4 * est[1], rtol=1e-5)
+
+
+@pytest.mark.parametrize("case", ["mid", "cfg3_plane", "cfg5_plane"])
+def test_a_bare_field_solve_keeps_the_nonlinear_bound(case):
+    # The diagnostics loop "step, gk_field_solve (for spectra / fluxes), gk_estimate_dt" must still see the bound of
+    # the step's last stage launch: only a field solve that a stage launch follows re-arms the maximum.
+    cfg, g = _ctx(case)
+    f = (0.05 * rand_c(np.random.default_rng(84), g.shape, True)).astype(np.complex64)
+    fd = g.to_state(f)
+    g.gk_rk4_steps(fd, 1e-3, 1)
+    before = g.gk_estimate_dt()
+    assert np.isfinite(before[1])
+    phi = g.gk_field_solve(fd)
+    g.gk_spectra(phi)
+    g.gk_fluxes(fd, phi)
+    assert np.array_equal(g.gk_estimate_dt(), before)
+    # gk_reset_cfl: back to the linear-only estimate, e.g. before the context is reused for another state
+    g.gk_reset_cfl()
+    after = g.gk_estimate_dt()
+    assert np.isinf(after[1]) and after[0] == min(before[2], before[3])
+    g.gk_rhs(fd)
+    assert np.isfinite(g.gk_estimate_dt()[1])
 
 
 def test_cfl_adaptive_steps_follow_the_lagged_estimate():
@@ -99,7 +124,7 @@ def test_cfl_adaptive_steps_follow_the_lagged_estimate():
 
 
 @pytest.mark.parametrize("case", ["mid", "mid_kinetic", "cfg2_plane", "cfg3_plane", "cfg3_plane_kinetic", "cfg5_plane",
-                                  "cfg3_plane_linear", "cfg5_plane_linear"])
+                                  "cfg3_plane_linear", "cfg5_plane_linear", "tiny_linear"])
 def test_fluxes_from_the_stage_epilogue(case):
     import torch
     from paper_2604_06085_b200 import GkError

@@ -153,7 +153,7 @@ def test_rk4_steps_parity_on_the_production_kernels(case):
     if case.endswith("_f16"):
         cfg["opts"]["storage"] = 1
     g = GkContext(cfg)
-    assert g.plan()["kind"] == kind or (kind == 3 and g.plan()["kind"] == 7), g.plan()
+    assert g.plan()["kind"] == kind, g.plan()
     o = GkRef(cfg)
     # white noise of amplitude 0.03 in every mode: the bracket is a few per cent of the increment and the three
     # steps stay bounded (amplitude 0.1 blows up within three steps, in the oracle as on the device)
@@ -196,7 +196,7 @@ def test_rhs_on_the_production_kernels_with_an_asymmetric_ky0_column(case):
         cfg["opts"]["nonlinear"] = 0
         kind = 3
     g, o = GkContext(cfg, full_workspace=False), GkRef(cfg)
-    assert g.plan()["kind"] == kind or (kind == 3 and g.plan()["kind"] == 7), g.plan()
+    assert g.plan()["kind"] == kind, g.plan()
     f = rand_c(np.random.default_rng(71), o.shape, False).astype(np.complex64)      # amplitude O(1): bracket ~ linear terms
     rhs, phi = g.gk_rhs(g.to_state(f))
     ref, phiref = o.rhs(f)
@@ -228,8 +228,8 @@ def test_rk4_parity_with_many_work_items_per_cta(case):
         kind = 3
     g, o = GkContext(cfg), GkRef(cfg)
     p = g.plan()
-    assert p["kind"] == kind or (kind == 3 and p["kind"] == 7), p
-    nsu = depth["ns"] if p["kind"] != 7 else (depth["ns"] + 7) // 8      # the tile kernel takes 8 s planes per item
+    assert p["kind"] == kind, p
+    nsu = depth["ns"]
     items = nsu * depth["nmu"] * p["nchunk"] * p["nsh"]
     assert items >= 3 * (p["stage_grid"] // p["cluster"]), (items, p)
     f = (rand_c(np.random.default_rng(72), o.shape, True) * 0.03).astype(np.complex64)
@@ -265,7 +265,7 @@ def test_config3_gradient_scan_on_the_production_kernel(rlt):
     cfg, kind = _plane_cfg("cfg3_plane")
     cfg["species"][0]["rlt"] = rlt
     g, o = GkContext(cfg), GkRef(cfg)
-    assert g.plan()["kind"] == kind or (kind == 3 and g.plan()["kind"] == 7)
+    assert g.plan()["kind"] == kind
     f = (rand_c(np.random.default_rng(73), o.shape, True) * 0.03).astype(np.complex64)
     fd = g.to_state(f)
     g.gk_rk4_steps(fd, 0.01, 3)
@@ -291,7 +291,7 @@ def test_half_storage_on_the_production_kernels(case):
         cfg["opts"]["nonlinear"] = 0
         kind = 3
     g = GkContext(cfg)
-    assert g.plan()["kind"] == kind or (kind == 3 and g.plan()["kind"] == 7)
+    assert g.plan()["kind"] == kind
     o = GkRef(cfg)
     f = (rand_c(np.random.default_rng(74), o.shape, True) * 0.03).astype(np.complex64)
     fd = g.to_state(f)
@@ -312,7 +312,7 @@ def test_fp16_storage_at_the_configured_amplitude():
     cfg["opts"]["storage"] = 1
     cfg["amp"], cfg["seed"] = 1e-3, 1239
     g, o = GkContext(cfg), GkRef(cfg)
-    assert g.plan()["kind"] == kind or (kind == 3 and g.plan()["kind"] == 7)
+    assert g.plan()["kind"] == kind
     f = gkinputs.initial_f(cfg, np.complex64)
     assert (np.abs(f.real) < 6.1e-5).mean() > 0.05          # the subnormal range is really exercised
     fd = g.to_state(f)
