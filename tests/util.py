@@ -34,6 +34,19 @@ def rel_l2(a, b):
     return float(np.linalg.norm((a - b).ravel()) / max(np.linalg.norm(b.ravel()), 1e-300))
 
 
+def max_abs_rel(a, b):
+    """max |a - b| / max |b|: a handful of wrong points (a seam row, an open-end class) cannot hide in it the way
+    they can in the relative L2 norm of 1e8 points."""
+    a = np.asarray(a)
+    b = np.asarray(b)
+    worst = 0.0
+    flat_a, flat_b = a.reshape(-1), b.reshape(-1)
+    step = 1 << 24                                   # chunked: no full-size temporaries at 6.7e7 points
+    for q in range(0, flat_a.size, step):
+        worst = max(worst, float(np.abs(flat_a[q:q + step] - flat_b[q:q + step]).max()))
+    return worst / max(float(np.abs(flat_b).max()), 1e-300)
+
+
 def rand_c(rng, shape, hermitian_ky0=True):
     z = rng.standard_normal(shape) + 1j * rng.standard_normal(shape)
     if hermitian_ky0:
