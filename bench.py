@@ -268,128 +268,159 @@ def run_reference(args, cfg, rank):
     print(json.dumps(line), flush=True)
 
 
-def run_cufft_compare(args, cfg):
-    """Measured comparisons only (north_star: cuFFT is allowed as a measured comparison).  Term III of one
-    stage done the library way, on arrays of the workload's (kx, ky) plane, beside the fused stage kernel:
+class LibraryBracket:
+    """Term III of one (kx, ky) slab batch the LIBRARY way (torch.fft = cuFFT on a CUDA device), kept as a measured
+    comparison (north_star) and checked against the oracle by tests/test_gpu_compare.py.
 
-      r2c     padded gradient spectra written to HBM, batched cuFFT c2r (torch.fft.irfft2) x 2 per slab, pointwise
-              product, cuFFT r2c, truncation (round 1's comparison; a timing of the data movement);
-      packed  the paper's own layout (D.3): both gradients of a field packed into ONE complex field
-              Z = d_x g + i d_y g, its full 2-D spectrum synthesised from the stored half by Hermitian extension with
-              the ky = 0 mirror pairs (kx, -kx) replaced by their Hermitian average, one C2C inverse per field, bracket,
-              one forward r2c; in complex64 (the paper's MP bracket) and in complex128 (its DP bracket).
+    This is an UNFUSED pipeline: padded spectra and real-space fields are materialised in HBM between torch ops.  It is
+    not the paper's design either: PAPER.md:420-426 fuses (1) scatter + i kx / i ky + J0 + scaling into the inverse
+    transform's load callback, (2) the bracket product into the forward transform's load callback and (3) the
+    truncation into its store callback; this pipeline has none of the three -- only the paper's data LAYOUT (the
+    two-for-one packing of D.3 with the Hermitian average of PAPER.md:440) is reproduced, in the `packed` leg.
 
-    The packed legs are CHECKED against the oracle's bracket (direct definition through its own FFT) on a few slabs
-    before they are timed, so the comparison is between two correct implementations of the same operation."""
+      r2c     both gradients of a field as separate half spectra, batched c2r inverse (which "discards the imaginary
+              output by construction", PAPER.md:438), pointwise product, r2c forward, truncation;
+      packed  Z = d_x g + i d_y g as ONE full complex spectrum (Hermitian extension; ky = 0 mirror pairs (kx, -kx)
+              replaced by their Hermitian average unless hermitian_average=False), one C2C inverse per field, bracket,
+              one r2c forward; complex64 (the paper's MP bracket) or complex128 (its DP bracket).
+    Inputs: half spectra [..., nkx, nky] (kx index -K..K, ky index 0..nky-1); output: the bracket
+    (1/2)(d_y chi d_x f - d_x chi d_y f), truncated to the retained modes, as the oracle's bracket_slab returns it."""
+
+    def __init__(self, nkx, nky, mx, my, dkx, ky0, device):
+        self.nkx, self.nky, self.mx, self.my, self.dkx, self.ky0, self.dev = nkx, nky, mx, my, dkx, ky0, device
+        self.K = (nkx - 1) // 2
+
+    def _k(self, rdt):
+        import torch
+        kx = ((torch.arange(self.nkx, device=self.dev) - self.K).to(rdt) * self.dkx).view(self.nkx, 1)
+        ky = (torch.arange(self.nky, device=self.dev).to(rdt) * self.ky0).view(1, self.nky)
+        return kx, ky
+
+    def _pad_half(self, src):
+        """[..., nkx, nky] -> zero-padded half spectrum [..., mx, my//2+1] in FFT order along kx."""
+        import torch
+        K, mx, nky = self.K, self.mx, self.nky
+        pad = torch.zeros(src.shape[:-2] + (mx, self.my // 2 + 1), dtype=src.dtype, device=self.dev)
+        pad[..., :K + 1, :nky] = src[..., K:, :]
+        pad[..., mx - K:, :nky] = src[..., :K, :]
+        return pad
+
+    def _truncate(self, out):
+        import torch
+        K, mx, nky = self.K, self.mx, self.nky
+        return torch.cat((out[..., mx - K:, :nky], out[..., :K + 1, :nky]), dim=-2)
+
+    def grad_real(self, gs):
+        """Real-space (d_x g, d_y g) on the padded grid through c2r transforms."""
+        import torch
+        kx, ky = self._k(torch.float64 if gs.dtype == torch.complex128 else torch.float32)
+        return (torch.fft.irfft2(self._pad_half(1j * kx * gs), s=(self.mx, self.my), norm="forward"),
+                torch.fft.irfft2(self._pad_half(1j * ky * gs), s=(self.mx, self.my), norm="forward"))
+
+    def r2c(self, fb, chib=None, gchi=None):
+        """gchi: real-space grad(chi) to reuse over vpar (as the paper and the fused kernel do), else built from chib."""
+        import torch
+        if gchi is None:
+            gchi = self.grad_real(chib)
+        fx, fy = self.grad_real(fb)
+        br = 0.5 * (gchi[1] * fx - gchi[0] * fy)
+        return self._truncate(torch.fft.rfft2(br, norm="forward"))
+
+    def packed_spectrum(self, gs, cdt, hermitian_average=True):
+        """Half spectrum -> full padded 2-D spectrum [..., mx, my] of d_x g + i d_y g."""
+        import torch
+        K, mx, my, nkx, nky = self.K, self.mx, self.my, self.nkx, self.nky
+        M = nky - 1
+        gs = gs.to(cdt)
+        kxv, kyv = self._k(torch.float64 if cdt == torch.complex128 else torch.float32)
+        g0 = gs.clone()
+        if hermitian_average:     # PAPER.md:440: both members of a ky = 0 mirror pair become their Hermitian average
+            g0[..., 0] = 0.5 * (gs[..., 0] + torch.conj(torch.flip(gs[..., 0], dims=(-1,))))
+        zp = (1j * kxv - kyv) * g0                                   # ky >= 0: (i kx) g + i (i ky) g
+        zm = torch.conj(torch.flip(g0, dims=(-2,)))                  # value at (kx, -ky) = conj g(-kx, ky)
+        zmm = (1j * kxv + kyv) * zm                                  # (i kx) g(kx,-ky) + i (i (-ky)) g(kx,-ky)
+        full = torch.zeros(gs.shape[:-2] + (mx, my), dtype=cdt, device=self.dev)
+        for lo, hi, dst in ((K, nkx, slice(0, K + 1)), (0, K, slice(mx - K, mx))):
+            full[..., dst, :nky] = zp[..., lo:hi, :]
+            if M > 0:
+                full[..., dst, my - M:] = torch.flip(zmm[..., lo:hi, 1:], dims=(-1,))
+        return full
+
+    def packed(self, fb, chib, cdt, hermitian_average=True, zc=None):
+        """zc: the C2C inverse of chi's packed spectrum to reuse over vpar, else built from chib."""
+        import torch
+        if zc is None:
+            zc = torch.fft.ifft2(self.packed_spectrum(chib, cdt, hermitian_average), norm="forward")
+        zf = torch.fft.ifft2(self.packed_spectrum(fb, cdt, hermitian_average), norm="forward")   # Re = d_x f, Im = d_y f
+        br = 0.5 * (zc.imag * zf.real - zc.real * zf.imag)
+        return self._truncate(torch.fft.rfft2(br, norm="backward") / (self.mx * self.my))
+
+
+def _time_cuda(fn, reps):
     import torch
-    from oracle.gkref import GkRef
-    from paper_2604_06085_b200 import GkContext
-    dev = torch.device("cuda", 0)
-    g = GkContext(cfg, device=dev)
+    for _ in range(2):
+        fn()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(reps):
+        fn()
+    e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) / reps
+
+
+def library_compare_block(g, cfg, batches=3):
+    """Bounded measurement for the bench line: `batches` batches of 4 (mu, s) pairs x nv slabs of the workload's plane
+    through the three library legs, extrapolated to the slabs of one stage (said so in the block).  grad(chi) / the
+    packed chi field are built once per batch and reused over vpar, as the fused kernel does."""
+    import torch
+    dev = g.device
     nsp, nv, nmu, ns, nkx, nky = g.shape
-    K = (nkx - 1) // 2
     plan = g.plan()
-    mx, my = plan["mx"], plan["my"]
-    M = nky - 1
-    dkx = float(g.gk_export_table("kx")[K + 1] - g.gk_export_table("kx")[K])
-    ky0 = cfg["grid"]["ky0"]
-    nli = 4                                   # (mu, s) pairs per batch: nli * nv slabs
+    kxt = g.gk_export_table("kx")
+    K = (nkx - 1) // 2
+    lb = LibraryBracket(nkx, nky, plan["mx"], plan["my"], float(kxt[K + 1] - kxt[K]), cfg["grid"]["ky0"], dev)
+    nli = 4
     nbatch = (nsp * nmu * ns + nli - 1) // nli
     gen = torch.Generator(device=dev).manual_seed(1)
     f = torch.view_as_complex(torch.randn(nli, nv, nkx, nky, 2, device=dev, generator=gen)) * 1e-3
     chi = torch.view_as_complex(torch.randn(nli, 1, nkx, nky, 2, device=dev, generator=gen)) * 1e-2
-    reps = max(1, args.steps)
+    scale = nbatch
+    out = {"what": "term III only (no linear terms, RK update or field solve) through torch.fft (cuFFT) as an UNFUSED "
+                   "library pipeline with padded arrays in HBM; not the paper's LTO-callback design (PAPER.md:420-426: "
+                   "none of its three callback fusions), only its packed-C2C layout with the Hermitian average "
+                   "(PAPER.md:428-442); parity of every leg against the oracle: tests/test_gpu_compare.py",
+           "padded_fft": [plan["mx"], plan["my"]], "slabs_per_stage": nsp * nv * nmu * ns,
+           "sample": f"{batches} timed batches of {nli * nv} slabs, extrapolated x{nbatch} to one stage"}
+    out["cufft_r2c_bracket_ms_per_stage"] = scale * _time_cuda(lambda: lb.r2c(f, chib=chi), batches)
+    out["cufft_packed_c2c_fp32_bracket_ms_per_stage"] = scale * _time_cuda(lambda: lb.packed(f, chi, torch.complex64), batches)
+    out["cufft_packed_c2c_fp64_bracket_ms_per_stage"] = scale * _time_cuda(lambda: lb.packed(f, chi, torch.complex128), batches)
+    del f, chi
+    torch.cuda.empty_cache()
+    return out
 
-    # ---- leg "r2c" (as in round 1) ----
-    kx = (torch.arange(nkx, device=dev) - K).float().view(1, 1, nkx, 1) * dkx
-    ky = torch.arange(nky, device=dev).float().view(1, 1, 1, nky) * ky0
-    gchi = torch.randn(2, nli, 1, mx, my, device=dev, generator=gen)   # real-space grad(chi), reused over vpar
-    pad = torch.zeros(2, nli, nv, mx, my // 2 + 1, dtype=torch.complex64, device=dev)
 
-    def bracket_r2c():
-        gx, gy = 1j * kx * f, 1j * ky * f
-        for q, src in enumerate((gx, gy)):
-            pad[q, :, :, :K + 1, :nky] = src[:, :, K:, :]
-            pad[q, :, :, mx - K:, :nky] = src[:, :, :K, :]
-        real = torch.fft.irfft2(pad, s=(mx, my), norm="forward")
-        br = gchi[1] * real[0] - gchi[0] * real[1]
-        out = torch.fft.rfft2(br, norm="forward")
-        return torch.cat((out[:, :, mx - K:, :nky], out[:, :, :K + 1, :nky]), dim=2)
-
-    # ---- leg "packed": Z = d_x g + i d_y g through one C2C inverse per field ----
-    def packed_spectrum(gs, cdt):
-        """gs [..., nkx, nky] half spectrum -> full padded 2-D spectrum [..., mx, my] of d_x g + i d_y g."""
-        gs = gs.to(cdt)
-        rdt = torch.float64 if cdt == torch.complex128 else torch.float32
-        kxv = ((torch.arange(nkx, device=dev) - K).to(rdt) * dkx).view(nkx, 1)
-        kyv = (torch.arange(nky, device=dev).to(rdt) * ky0).view(1, nky)
-        g0 = gs.clone()
-        g0[..., 0] = 0.5 * (gs[..., 0] + torch.conj(torch.flip(gs[..., 0], dims=(-1,))))   # Hermitian average of the mirror pairs
-        zp = (1j * kxv - kyv) * g0                                   # ky >= 0:  (i kx) g + i (i ky) g
-        zm = torch.conj(torch.flip(g0, dims=(-2,)))                  # g(-kx... ) : value at (kx, -ky) = conj g(-kx, ky)
-        zmm = (1j * kxv + kyv) * zm                                  # (i kx) g(kx,-ky) + i (i (-ky)) g(kx,-ky)
-        full = torch.zeros(gs.shape[:-2] + (mx, my), dtype=cdt, device=dev)
-        for lo, hi, dst in ((K, nkx, slice(0, K + 1)), (0, K, slice(mx - K, mx))):
-            full[..., dst, :nky] = zp[..., lo:hi, :]
-            full[..., dst, my - M:] = torch.flip(zmm[..., lo:hi, 1:], dims=(-1,))
-        return full
-
-    def bracket_packed(fb, chib, cdt):
-        zf = torch.fft.ifft2(packed_spectrum(fb, cdt), norm="forward")       # Re = d_x f, Im = d_y f
-        zc = torch.fft.ifft2(packed_spectrum(chib, cdt), norm="forward")
-        br = 0.5 * (zc.imag * zf.real - zc.real * zf.imag)
-        out = torch.fft.rfft2(br, norm="backward") / (mx * my)
-        return torch.cat((out[..., mx - K:, :nky], out[..., :K + 1, :nky]), dim=-2)
-
-    # parity of the packed legs against the oracle's bracket, asymmetric ky = 0 columns included
-    o = GkRef(cfg, pad=(mx, my))
-    rng = np.random.default_rng(5)
-    fs = (rng.standard_normal((3, nkx, nky)) + 1j * rng.standard_normal((3, nkx, nky)))
-    cs = (rng.standard_normal((3, nkx, nky)) + 1j * rng.standard_normal((3, nkx, nky)))
-    parity = {}
-    for name, cdt in (("packed_c64", torch.complex64), ("packed_c128", torch.complex128)):
-        got = bracket_packed(torch.from_numpy(fs).to(dev), torch.from_numpy(cs).to(dev), cdt).cpu().numpy()
-        ref = np.stack([o.bracket_slab(cs[q], fs[q], 0, mx, my) for q in range(3)])
-        parity[name] = float(np.linalg.norm(got - ref) / np.linalg.norm(ref))
-    assert parity["packed_c64"] < 1e-5 and parity["packed_c128"] < 1e-12, parity
-
-    def time_leg(fn):
-        for _ in range(3):
-            fn()
-        torch.cuda.synchronize()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record()
-        for _ in range(reps * nbatch):
-            fn()
-        e1.record()
-        torch.cuda.synchronize()
-        return e0.elapsed_time(e1) / reps
-
-    ms_r2c = time_leg(bracket_r2c)
-    ms_p64 = time_leg(lambda: bracket_packed(f, chi, torch.complex64))
-    ms_p128 = time_leg(lambda: bracket_packed(f, chi, torch.complex128))
-    # the fused stage kernel (whole stage: field solve + linear terms + bracket + RK update) on the same grid
+def run_cufft_compare(args, cfg):
+    """`--compare cufft`: the library legs timed over ALL slabs of a stage (no extrapolation) beside the fused stage."""
+    import torch
+    from paper_2604_06085_b200 import GkContext
+    dev = torch.device("cuda", 0)
+    g = GkContext(cfg, device=dev)
+    nsp, nv, nmu, ns, nkx, nky = g.shape
+    nbatch = (nsp * nmu * ns + 3) // 4
+    blk = library_compare_block(g, cfg, batches=max(1, args.steps) * nbatch)
+    blk["sample"] = f"every slab of {max(1, args.steps)} stage(s), no extrapolation"
     fd = g.to_state(gkinputs.initial_f(cfg, np.complex64))
     g.gk_rk4_steps(fd, cfg["dt"], 3)
     torch.cuda.synchronize()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
-    g.gk_rk4_steps(fd, cfg["dt"], reps)
+    g.gk_rk4_steps(fd, cfg["dt"], max(1, args.steps))
     e1.record()
     torch.cuda.synchronize()
-    fused = e0.elapsed_time(e1) / (4 * reps)
-    print(json.dumps({"compare": "cufft_bracket", "workload": cfg["name"], "padded_fft": [mx, my],
-                      "slabs_per_stage": nsp * nv * nmu * ns, "batch_slabs": nli * nv,
-                      "cufft_r2c_bracket_ms_per_stage": ms_r2c,
-                      "cufft_packed_c2c_fp32_bracket_ms_per_stage": ms_p64,
-                      "cufft_packed_c2c_fp64_bracket_ms_per_stage": ms_p128,
-                      "packed_parity_vs_oracle_rel_l2": parity,
-                      "fused_whole_stage_ms": fused,
-                      "ratio_packed_fp32_bracket_over_whole_fused_stage": ms_p64 / fused,
-                      "note": "torch.fft (cuFFT) with padded arrays in HBM; term III only (no linear terms, no RK update, "
-                              "no field solve); the packed legs build the full Hermitian-extended spectrum with the "
-                              "mirror-pair average of PAPER.md:440 and pass a parity check against the oracle first"}),
-          flush=True)
+    blk["fused_whole_stage_ms"] = e0.elapsed_time(e1) / (4 * max(1, args.steps))
+    print(json.dumps({"compare": "cufft_bracket", "workload": cfg["name"], **blk}), flush=True)
 
 
 def main():
@@ -404,6 +435,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs)")
     ap.add_argument("--no-secondary", action="store_true", help="skip the config-3 stage timing that follows a config-5 run")
+    ap.add_argument("--no-compare", action="store_true", help="skip the bounded cuFFT comparison block of the bench line")
     ap.add_argument("--compare", default=None, choices=["cufft"], help="measured comparison: term III through cuFFT, unfused")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "gk" else args.warmup
@@ -513,6 +545,11 @@ def main():
     plan = g.plan()
     kernel_names = {0: "gk_stage_kernel", 2: "gk_stage_ws2_kernel", 3: "gk_stage_lin_kernel", 5: "gk_stage_ws4_kernel", 6: "gk_stage_point_kernel"}
 
+    # ---- the library formulation of term III beside the fused stage, after the timed regions ----
+    compare = None
+    if rank == 0 and world == 1 and nl and not args.no_compare:
+        compare = library_compare_block(g, cfg, batches=3)
+
     # ---- secondary workload (rank 0, N = 1): the stage kernel of BASELINE config 3 (the round-1 headline) ----
     secondary = None
     if rank == 0 and world == 1 and args.config == 5 and not args.no_secondary:
@@ -552,7 +589,9 @@ def main():
                                   "smem": plan["stage_smem"], "vpar_chunks": plan["nchunk"]},
                        "l2": "inputs larger than L2 (state + 3 work arrays)" if npts * 8 * 4 > 126e6 * 2
                        else "working set comparable to L2; not flushed",
-                       "parallelism": "replicas only (paper has no grid parallelism)", "finite": finite},
+                       "parallelism": "replicas only (paper has no grid parallelism)", "finite": finite,
+                       # readings no number of the authors can pin (oracle/gkref.h header)
+                       "unpinned_readings": ["R7", "R9", "R18"]},
             "step_ms": {"median": float(np.median(per_step)), "min": float(np.min(per_step)),
                         "max": float(np.max(per_step)), "repetitions": len(per_step)},
             "clocks": clocks,
@@ -567,6 +606,9 @@ def main():
         }
         if secondary:
             line["secondary"] = secondary
+        if compare:
+            compare["fused_whole_stage_ms"] = roof["avg_launch_ms"]
+            line["compare"] = compare
         if not args.no_cpu_baseline and world == 1:
             line["cpu_baseline"] = _oracle_sample(cfg, budget_s=12.0)
         print(json.dumps(line), flush=True)
