@@ -158,8 +158,12 @@ def test_rosenbluth_hinton_residual():
     # disp_par=0.01, zonal initial condition: phi(inf)/phi(0) = 1/(1+q^2 Theta/eps^2) = 0.07105.
     # Reduced resolution and run time (the paper uses 128x128x16 to t=100 and quotes 0.1 %): the
     # GAM (omega ~ 2.07 v_th/R, weakly damped at q=1.3) is removed by averaging over whole periods.
+    # The v_par grid is the paper's (Nv = 128): DESIGN.md section 4 shows that the v_par resolution is the one knob
+    # the residual depends on (recurrence time 2 pi q R / dv = 131 at Nv = 128; t = 60 stays below half of it), while
+    # Ns = 32 and Nmu = 8 cost well under a per cent.  Measured: 0.07202 (+1.4 %); the round-1 grid 16 x 48 x 8
+    # (recurrence at t = 49, inside the averaging window) gave -5.9 % and needed a 12 % tolerance.
     q, shat, eps = 1.3, 0.1592, 0.05
-    cfg = small_cfg(nkx=3, nky=1, ns=16, nvpar=48, nmu=8, mu_grid=1, ky0=0.025 / (2 * np.pi * shat),
+    cfg = small_cfg(nkx=3, nky=1, ns=32, nvpar=128, nmu=8, mu_grid=1, ky0=0.025 / (2 * np.pi * shat),
                     ikxspace=1, nonlinear=0, disp_par=0.01, disp_vp=0.0, disp_x=0.0, disp_y=0.0)
     cfg["geom"].update(q=q, shat=shat, eps=eps)
     cfg["species"][0].update(rlt=0.0, rln=0.0)
@@ -190,4 +194,4 @@ def test_rosenbluth_hinton_residual():
     nper = 6
     win = (t > 60 - nper * period)
     resid = tr[win].mean()
-    assert abs(resid - theory) < 0.12 * theory, (resid, theory)
+    assert abs(resid - theory) < 0.05 * theory, (resid, theory)
