@@ -358,7 +358,7 @@ class LibraryBracket:
 
 def _time_cuda(fn, reps):
     import torch
-    for _ in range(2):
+    for _ in range(3):          # cuFFT plan creation and the caching allocator's first blocks stay outside
         fn()
     torch.cuda.synchronize()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -370,7 +370,7 @@ def _time_cuda(fn, reps):
     return e0.elapsed_time(e1) / reps
 
 
-def library_compare_block(g, cfg, batches=3):
+def library_compare_block(g, cfg, batches=10):
     """Bounded measurement for the bench line: `batches` batches of 4 (mu, s) pairs x nv slabs of the workload's plane
     through the three library legs, extrapolated to the slabs of one stage (said so in the block).  grad(chi) / the
     packed chi field are built once per batch and reused over vpar, as the fused kernel does."""
@@ -548,7 +548,7 @@ def main():
     # ---- the library formulation of term III beside the fused stage, after the timed regions ----
     compare = None
     if rank == 0 and world == 1 and nl and not args.no_compare:
-        compare = library_compare_block(g, cfg, batches=3)
+        compare = library_compare_block(g, cfg)
 
     # ---- secondary workload (rank 0, N = 1): the stage kernel of BASELINE config 3 (the round-1 headline) ----
     secondary = None

@@ -14,13 +14,14 @@ def rh_theory(q, eps):
     return 1.0 / (1.0 + q * q * theta / eps ** 2)
 
 
-def run_rh(eps, ns=128, nv=128, nmu=16, t_end=100.0, dt=0.01, blk=10):
-    """phi(t)/phi(0) of the kx = +dkx zonal mode, flux-surface averaged, every blk steps."""
+def run_rh(eps, ns=128, nv=128, nmu=16, t_end=100.0, dt=0.01, blk=10, disp_par=0.01, disp_vp=0.0, **grid_kw):
+    """phi(t)/phi(0) of the kx = +dkx zonal mode, flux-surface averaged, every blk steps.  grid_kw: vpar_max,
+    vperp_max (the convergence table of DESIGN.md section 4)."""
     import torch
     from paper_2604_06085_b200 import GkContext
     q, shat = 1.3, 0.1592
     cfg = small_cfg(nkx=3, nky=1, ns=ns, nvpar=nv, nmu=nmu, mu_grid=1, ky0=0.025 / (2 * np.pi * shat), ikxspace=1,
-                    nonlinear=0, disp_par=0.01, disp_vp=0.0, disp_x=0.0, disp_y=0.0)
+                    nonlinear=0, disp_par=disp_par, disp_vp=disp_vp, disp_x=0.0, disp_y=0.0, **grid_kw)
     cfg["geom"].update(q=q, shat=shat, eps=eps)
     cfg["species"][0].update(rlt=0.0, rln=0.0)
     g = GkContext(cfg)
@@ -61,7 +62,23 @@ def test_rosenbluth_hinton_residual_at_the_papers_resolution():
     # GAM frequency (fluid theory with the finite-q correction, as in tests/test_oracle_physics.py)
     np.testing.assert_allclose(omega, np.sqrt(7 / 4 + 1) * np.sqrt(1 + 46 / (49 * q * q)), rtol=0.03)
     print(f"RH eps=0.05: residual {res:.5f} (fit constant {const:.5f}) theory {theory:.5f} ratio {res / theory:.4f} omega_GAM {omega:.4f}")
-    assert abs(res / theory - 1) < 0.03, (res, theory)
+    # measured 1.0096; DESIGN.md section 4 (convergence table): the +1 % is the v_par resolution (recurrence time
+    # 2 pi q R / dv = 131 at Nv = 128, not far beyond t = 100), every other knob moves the residual by <= 0.2 %
+    assert abs(res / theory - 1) < 0.015, (res, theory)
+
+
+def test_rosenbluth_hinton_residual_converges_in_vpar_resolution():
+    # the same case at Nv = 256 (recurrence time 262): the paper's "0.1 %" level; measured +0.13 %
+    t, tr, q = run_rh(0.05, nv=256)
+    res, _, _ = residual(t, tr, q)
+    theory = rh_theory(q, 0.05)
+    print(f"RH eps=0.05 Nv=256: residual {res:.5f} theory {theory:.5f} ratio {res / theory:.4f}")
+    assert abs(res / theory - 1) < 0.005, (res, theory)
+
+
+# measured ratios to eq. 5 at the paper's resolution; the growing offset is the accuracy of the
+# small-eps expansion itself (at eps = 0.25: +3.0 % at Nv = 256, +2.1 % at Nv = 512)
+RH_SCAN = {0.10: 1.010, 0.15: 1.019, 0.20: 1.028, 0.25: 1.034}
 
 
 @pytest.mark.parametrize("eps", [0.10, 0.15, 0.20, 0.25])
@@ -71,7 +88,8 @@ def test_rosenbluth_hinton_epsilon_scan(eps):
     res, omega, const = residual(t, tr, q)
     theory = rh_theory(q, eps)
     print(f"RH eps={eps}: residual {res:.5f} (fit constant {const:.5f}) theory {theory:.5f} ratio {res / theory:.4f}")
-    assert abs(res / theory - 1) < 0.06, (res, theory)
+    assert abs(res / theory - RH_SCAN[eps]) < 0.006, (res, theory)      # what is achieved, plus a small margin
+    assert abs(res / theory - 1) < 0.04, (res, theory)
 
 
 # ---- Cyclone base case, linear ITG: q = 1.4, shat = 0.78, eps = 0.19, R/LT = 6.9, R/Ln = 2.2,

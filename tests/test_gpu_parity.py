@@ -7,7 +7,7 @@ import pytest
 import gkinputs
 from oracle import gkref as G
 from oracle.gkref import GkRef
-from tests.util import small_cfg, rand_c, rel_l2
+from tests.util import max_abs_rel, small_cfg, rand_c, rel_l2
 
 pytestmark = pytest.mark.gpu
 
@@ -64,6 +64,7 @@ def test_rhs_parity_one_term_at_a_time(bit):
     ref, _ = o.rhs(f)
     assert np.linalg.norm(ref) > 0
     assert rel_l2(rhs.cpu().numpy(), ref) < TOL_RHS, bit
+    assert max_abs_rel(rhs.cpu().numpy(), ref) < 1e-4, bit
 
 
 @pytest.mark.parametrize("case", ["cfg1", "mid", "mid2", "mid_kinetic", "closure1", "tiny"])
@@ -79,6 +80,7 @@ def test_rhs_parity_full(case):
     ref, phiref = o.rhs(f)
     assert rel_l2(phi.cpu().numpy(), phiref) < TOL_RHS
     assert rel_l2(rhs.cpu().numpy(), ref) < TOL_RHS
+    assert max_abs_rel(rhs.cpu().numpy(), ref) < 1e-4
 
 
 @pytest.mark.parametrize("case,kind", [("chain", 6), ("mid", 6), ("mid2", 0), ("mid_kinetic", 6)])
@@ -95,6 +97,7 @@ def test_linear_runs_on_the_point_and_generic_kernels(case, kind):
     ref, phiref = o.rhs(f)
     assert rel_l2(phi.cpu().numpy(), phiref) < TOL_RHS
     assert rel_l2(rhs.cpu().numpy(), ref) < TOL_RHS
+    assert max_abs_rel(rhs.cpu().numpy(), ref) < 1e-4
     dt = 0.0005 if case == "mid_kinetic" else 0.01
     fd = g.to_state(f)
     g.gk_rk4_steps(fd, dt, 10)
@@ -304,6 +307,7 @@ def test_circular_geometry_rhs_steps_fluxes_and_cfl(case):
     ref, phiref = o.rhs(f)
     assert rel_l2(phi.cpu().numpy(), phiref) < TOL_RHS
     assert rel_l2(rhs.cpu().numpy(), ref) < TOL_RHS
+    assert max_abs_rel(rhs.cpu().numpy(), ref) < 1e-4
     est, eref = g.gk_estimate_dt(), o.estimate_dt(phi.cpu().numpy().astype(np.complex128))
     for k in range(4):
         if np.isinf(eref[k]):
